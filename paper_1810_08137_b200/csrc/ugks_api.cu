@@ -1,0 +1,306 @@
+// ugks_api.cu -- the C ABI of include/ugks.h: context, workspace carving, launch sequencing.
+#include "../../include/ugks.h"
+#include "ugks_common.cuh"
+
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+struct ugks_ctx {
+    UgksParams P;
+    cudaStream_t st;
+    int cur;                  // which of f[2] / W[2] holds the current state
+    int have_state, have_res;
+    long steps, launches;
+    int resblocks, nchunk_alloc;
+    double *res_dev, *bcprim_dev, *Wf_dev;
+    double *ghost, *wallg, *Wb, *wallG;     // non-const aliases of the P fields
+    size_t cells;
+    char err[256];
+};
+
+static char g_err[256] = "";
+static int fail(ugks_ctx *c, int code, const char *fmt, const char *detail)
+{
+    char *dst = c ? c->err : g_err;
+    snprintf(dst, 256, fmt, detail ? detail : "");
+    return code;
+}
+static int cuda_fail(ugks_ctx *c, cudaError_t e, const char *where)
+{
+    char buf[200];
+    snprintf(buf, sizeof buf, "%s: %s", where, cudaGetErrorString(e));
+    return fail(c, UGKS_ECUDA, "CUDA error in %s", buf);
+}
+#define CK(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, where); } while (0)
+
+static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// launch geometry heuristics: chunk of velocity rows sized for shared memory,
+// R rows in parallel so that blockDim = Nu*R ~ 128..256 threads, strip length for >= ~4 CTAs per SM
+static void choose_geometry(int I, int J, int Nu, int Nv, int *chunk_m, int *R, int *strip)
+{
+    int cm = 800 / Nu; if (cm < 1) cm = 1;
+    if (cm >= Nv) cm = Nv;
+    else if ((Nu & 1) && (cm & 1)) cm += 1;                 // 16-byte aligned chunk starts for odd Nu
+    int rmax = 256 / Nu; if (rmax < 1) rmax = 1; if (rmax > cm) rmax = cm;
+    int r = rmax;
+    for (int t = rmax; t >= 1 && 2 * t >= rmax; --t) if (cm % t == 0) { r = t; break; }
+    *chunk_m = cm; *R = r;
+    const int nchunk = (Nv + cm - 1) / cm;
+    int s = 32;
+    while (s > 8 && (long)J * ((I + s - 1) / s) * nchunk < 148L * 4) s >>= 1;
+    *strip = s;
+}
+
+struct Layout {
+    size_t f[2], W[2], mom[2], coef[2], fw[2], cellc, respart, res, status, u, wu, v, wv, ghost, wallg, Wb, wallG,
+        bcprim, Wf, total;
+    int Npad, resblocks, nchunk_alloc;
+};
+static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
+{
+    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > 1024 || vg->Nv < 1) return 1;
+    const size_t cells = (size_t)m->I * m->J, N = (size_t)vg->Nu * vg->Nv;
+    const size_t Npad = (N + 15) & ~(size_t)15;
+    const size_t nfx = (size_t)(m->I + 1) * m->J, nfy = (size_t)m->I * (m->J + 1);
+    int cm, R, strip;
+    choose_geometry(m->I, m->J, vg->Nu, vg->Nv, &cm, &R, &strip);
+    const int nchunk = (vg->Nv + cm - 1) / cm;
+    L->nchunk_alloc = nchunk * 2;
+    L->Npad = (int)Npad;
+    L->resblocks = (int)((cells + 127) / 128);
+    size_t o = 0;
+#define TAKE(field, bytes) do { L->field = o; o += al256(bytes); } while (0)
+    TAKE(f[0], cells * Npad * 8); TAKE(f[1], cells * Npad * 8);
+    TAKE(W[0], cells * 32); TAKE(W[1], cells * 32);
+    TAKE(mom[0], nfx * L->nchunk_alloc * NMOM * 8); TAKE(mom[1], nfy * L->nchunk_alloc * NMOM * 8);
+    TAKE(coef[0], nfx * NCOEF * 8); TAKE(coef[1], nfy * NCOEF * 8);
+    TAKE(fw[0], nfx * 32); TAKE(fw[1], nfy * 32);
+    TAKE(cellc, cells * NCELL * 8);
+    TAKE(respart, (size_t)L->resblocks * 64);
+    TAKE(res, 64); TAKE(status, 64);
+    TAKE(u, vg->Nu * 8); TAKE(wu, vg->Nu * 8); TAKE(v, vg->Nv * 8); TAKE(wv, vg->Nv * 8);
+    TAKE(ghost, 4 * Npad * 8); TAKE(wallg, 4 * Npad * 8);
+    TAKE(Wb, 128); TAKE(wallG, 128); TAKE(bcprim, 128);
+    TAKE(Wf, cells * 32);
+#undef TAKE
+    L->total = o;
+    return 0;
+}
+
+extern "C" {
+
+const char *ugks_version(void) { return "ugks-b200 0.1 (sm_100a, fp64)"; }
+const char *ugks_last_error(const ugks_ctx *c) { return c ? c->err : g_err; }
+
+size_t ugks_workspace_bytes(const ugks_mesh *m, const ugks_vgrid *vg)
+{
+    Layout L;
+    return make_layout(m, vg, &L) ? 0 : L.total;
+}
+
+int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ugks_gas *gas, const ugks_bcs *bcs,
+              double cfl, void *workspace_dev, size_t workspace_bytes, void *cuda_stream)
+{
+    ugks_ctx *c = nullptr;
+    if (!out) return fail(c, UGKS_EINVAL, "%s", "out is NULL");
+    *out = nullptr;
+    if (!m || !vg || !gas || !bcs || !workspace_dev) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
+    Layout L;
+    if (make_layout(m, vg, &L)) return fail(c, UGKS_EINVAL, "%s", "invalid mesh or velocity grid size (I,J >= 2; 1 <= Nu <= 1024)");
+    if (!(m->x1 > m->x0) || !(m->y1 > m->y0)) return fail(c, UGKS_EINVAL, "%s", "empty domain");
+    if (!vg->u || !vg->wu || !vg->v || !vg->wv) return fail(c, UGKS_EINVAL, "%s", "NULL velocity arrays");
+    if (gas->Pr != 1.0) return fail(c, UGKS_EINVAL, "%s", "Pr must be 1 (BGK)");
+    if (gas->K_int != 0) return fail(c, UGKS_EINVAL, "%s", "K_int must be 0");
+    if (!(cfl > 0.0)) return fail(c, UGKS_EINVAL, "%s", "cfl must be positive");
+    const ugks_bc *b[4] = { &bcs->xmin, &bcs->xmax, &bcs->ymin, &bcs->ymax };
+    for (int s = 0; s < 4; ++s) {
+        if (b[s]->type < 0 || b[s]->type > 2) return fail(c, UGKS_EINVAL, "%s", "unknown boundary type");
+        if (b[s]->type != UGKS_BC_PERIODIC && !(b[s]->T > 0.0)) return fail(c, UGKS_EINVAL, "%s", "boundary T must be positive");
+        if (b[s]->type == UGKS_BC_FIXED && !(b[s]->rho > 0.0)) return fail(c, UGKS_EINVAL, "%s", "boundary rho must be positive");
+    }
+    if ((b[0]->type == UGKS_BC_PERIODIC) != (b[1]->type == UGKS_BC_PERIODIC) ||
+        (b[2]->type == UGKS_BC_PERIODIC) != (b[3]->type == UGKS_BC_PERIODIC))
+        return fail(c, UGKS_EINVAL, "%s", "periodic sides must be paired");
+    double swu = 0, swv = 0, umax = 0, vmax = 0;
+    for (int k = 0; k < vg->Nu; ++k) { swu += vg->wu[k]; umax = fmax(umax, fabs(vg->u[k])); }
+    for (int k = 0; k < vg->Nv; ++k) { swv += vg->wv[k]; vmax = fmax(vmax, fabs(vg->v[k])); }
+    if (!(swu > 0.0) || !(swv > 0.0) || !(umax + vmax > 0.0)) return fail(c, UGKS_EINVAL, "%s", "velocity weights/nodes degenerate");
+    if (workspace_bytes < L.total) return fail(c, UGKS_ENOMEM, "%s", "workspace smaller than ugks_workspace_bytes()");
+    if (((uintptr_t)workspace_dev & 255) != 0) return fail(c, UGKS_EINVAL, "%s", "workspace must be 256-byte aligned");
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(c, UGKS_ECUDA, "%s", "no CUDA device: libugks has no CPU fallback");
+    }
+    c = (ugks_ctx *)calloc(1, sizeof *c);
+    if (!c) return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed");
+    UgksParams &P = c->P;
+    P.I = m->I; P.J = m->J; P.Nu = vg->Nu; P.Nv = vg->Nv; P.N = vg->Nu * vg->Nv; P.Npad = L.Npad;
+    P.dx = (m->x1 - m->x0) / m->I; P.dy = (m->y1 - m->y0) / m->J;
+    P.dt = cfl / (umax / P.dx + vmax / P.dy);                                   // AMB-6
+    P.omega = gas->omega;
+    if (gas->mu_ref > 0.0) P.mu_ref = gas->mu_ref;
+    else {                                                                        // AMB-7, alpha = 1
+        const double al = 1.0;
+        P.mu_ref = 5.0 * (al + 1.0) * (al + 2.0) * sqrt(UGKS_PI) / (4.0 * al * (5.0 - 2.0 * gas->omega) * (7.0 - 2.0 * gas->omega)) * gas->Kn;
+    }
+    if (!(P.mu_ref > 0.0)) { free(c); return fail(nullptr, UGKS_EINVAL, "%s", "mu_ref / Kn must be positive"); }
+    for (int s = 0; s < 4; ++s) P.bc[s] = b[s]->type;
+    char *base = (char *)workspace_dev;
+    auto D = [&](size_t off) { return (double *)(base + off); };
+    P.f[0] = D(L.f[0]); P.f[1] = D(L.f[1]); P.W[0] = D(L.W[0]); P.W[1] = D(L.W[1]);
+    P.mom[0] = D(L.mom[0]); P.mom[1] = D(L.mom[1]); P.coef[0] = D(L.coef[0]); P.coef[1] = D(L.coef[1]);
+    P.fw[0] = D(L.fw[0]); P.fw[1] = D(L.fw[1]); P.cellc = D(L.cellc); P.respart = D(L.respart);
+    P.status = (int *)(base + L.status);
+    P.u = D(L.u); P.wu = D(L.wu); P.v = D(L.v); P.wv = D(L.wv);
+    c->ghost = D(L.ghost); c->wallg = D(L.wallg); c->Wb = D(L.Wb); c->wallG = D(L.wallG);
+    P.ghost = c->ghost; P.wallg = c->wallg; P.Wb = c->Wb; P.wallG = c->wallG;
+    c->res_dev = D(L.res); c->bcprim_dev = D(L.bcprim); c->Wf_dev = D(L.Wf);
+    c->resblocks = L.resblocks; c->nchunk_alloc = L.nchunk_alloc;
+    c->cells = (size_t)m->I * m->J;
+    c->st = (cudaStream_t)cuda_stream;
+    choose_geometry(P.I, P.J, P.Nu, P.Nv, &P.chunk_m, &P.R, &P.strip);
+    P.nchunk = (P.Nv + P.chunk_m - 1) / P.chunk_m;
+
+    double bcprim[16];
+    for (int s = 0; s < 4; ++s) { bcprim[s * 4] = b[s]->rho; bcprim[s * 4 + 1] = b[s]->U; bcprim[s * 4 + 2] = b[s]->V; bcprim[s * 4 + 3] = b[s]->T; }
+    cudaError_t e = cudaSuccess;
+    const struct { const double *src; size_t off; size_t n; } cp[5] = {
+        { vg->u, L.u, (size_t)vg->Nu }, { vg->wu, L.wu, (size_t)vg->Nu }, { vg->v, L.v, (size_t)vg->Nv },
+        { vg->wv, L.wv, (size_t)vg->Nv }, { bcprim, L.bcprim, 16 } };
+    for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaMemcpyAsync(base + cp[i].off, cp[i].src, cp[i].n * 8, cudaMemcpyHostToDevice, c->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(P.f[0], 0, c->cells * P.Npad * 8, c->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(P.f[1], 0, c->cells * P.Npad * 8, c->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(P.status, 0, 64, c->st);
+    if (e == cudaSuccess) { c->launches += launch_setup(P, c->bcprim_dev, c->ghost, c->wallg, c->Wb, c->wallG, c->st); e = cudaGetLastError(); }
+    if (e == cudaSuccess && (setup_moments_attributes(P) || setup_update_attributes(P))) e = cudaGetLastError() == cudaSuccess ? cudaErrorInvalidValue : cudaErrorInvalidValue;
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); free(c); return rc; }
+    *out = c;
+    return UGKS_OK;
+}
+
+void ugks_destroy(ugks_ctx *c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->st);
+    free(c);
+}
+
+double ugks_dt(const ugks_ctx *c) { return c ? c->P.dt : 0.0; }
+double ugks_mu_ref(const ugks_ctx *c) { return c ? c->P.mu_ref : 0.0; }
+long ugks_step_count(const ugks_ctx *c) { return c ? c->steps : -1; }
+long ugks_launch_count(const ugks_ctx *c) { return c ? c->launches : -1; }
+
+int ugks_set_option(ugks_ctx *c, const char *name, int value)
+{
+    if (!c || !name) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
+    UgksParams &P = c->P;
+    if (!strcmp(name, "strip")) {
+        if (value < 1 || value > 4096) return fail(c, UGKS_EINVAL, "%s", "strip out of range");
+        P.strip = value;
+        return UGKS_OK;
+    }
+    if (!strcmp(name, "chunk_m") || !strcmp(name, "R")) {
+        int cm = P.chunk_m, R = P.R;
+        if (!strcmp(name, "chunk_m")) cm = value; else R = value;
+        if (cm < 1 || cm > P.Nv || R < 1 || R > cm || P.Nu * R > 1024) return fail(c, UGKS_EINVAL, "%s", "chunk_m / R out of range");
+        const int nchunk = (P.Nv + cm - 1) / cm;
+        if (nchunk > c->nchunk_alloc) return fail(c, UGKS_EINVAL, "%s", "chunk_m too small for the allocated moment buffers");
+        if (nchunk > 1 && ((cm * P.Nu) & 1)) return fail(c, UGKS_EINVAL, "%s", "chunk_m * Nu must be even (16-byte aligned chunks)");
+        UgksParams T = P; T.chunk_m = cm; T.R = R; T.nchunk = nchunk;
+        if (smem_flux_update(T) > 227 * 1024) return fail(c, UGKS_EINVAL, "%s", "chunk does not fit in shared memory");
+        P = T;
+        if (setup_moments_attributes(P) || setup_update_attributes(P)) return cuda_fail(c, cudaGetLastError(), "ugks_set_option");
+        return UGKS_OK;
+    }
+    return fail(c, UGKS_EINVAL, "unknown option %s", name);
+}
+
+static int check_deferred(ugks_ctx *c, const char *where)
+{
+    CK(cudaStreamSynchronize(c->st), where);
+    CK(cudaGetLastError(), where);
+    int status[2] = { 0, 0 };
+    CK(cudaMemcpy(status, c->P.status, sizeof status, cudaMemcpyDeviceToHost), where);
+    if (status[0]) return fail(c, UGKS_ESTATE, "%s", "non-physical state (rho <= 0, lambda <= 0 or NaN) met during ugks_step");
+    return UGKS_OK;
+}
+
+int ugks_set_state(ugks_ctx *c, const double *W, const double *f, int on_dev)
+{
+    if (!c || !W || !f) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
+    const UgksParams &P = c->P;
+    const cudaMemcpyKind kind = on_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    c->cur = 0;
+    CK(cudaMemcpyAsync(P.W[0], W, c->cells * 32, kind, c->st), "ugks_set_state(W)");
+    CK(cudaMemcpy2DAsync(P.f[0], (size_t)P.Npad * 8, f, (size_t)P.N * 8, (size_t)P.N * 8, c->cells, kind, c->st), "ugks_set_state(f)");
+    CK(cudaMemsetAsync(P.status, 0, 64, c->st), "ugks_set_state");
+    if (!on_dev) CK(cudaStreamSynchronize(c->st), "ugks_set_state");
+    c->have_state = 1; c->have_res = 0; c->steps = 0;
+    return UGKS_OK;
+}
+
+int ugks_step(ugks_ctx *c, int n)
+{
+    if (!c || n < 0) return fail(c, UGKS_EINVAL, "%s", "bad argument");
+    if (!c->have_state) return fail(c, UGKS_ESTATE, "%s", "ugks_step before ugks_set_state");
+    for (int s = 0; s < n; ++s) {
+        c->launches += launch_face_moments(c->P, c->cur, c->st);       // R, S1, S7 sums
+        c->launches += launch_face_scalars(c->P, c->cur, c->st);       // S2..S5, wall density
+        c->launches += launch_cell_scalars(c->P, c->cur, c->resblocks, c->st);   // U1, U2, residual partials
+        c->launches += launch_flux_update(c->P, c->cur, c->st);        // S6, S8, U3
+        c->cur ^= 1;
+        c->steps += 1;
+    }
+    CK(cudaGetLastError(), "ugks_step");
+    if (n > 0) c->have_res = 1;
+    return UGKS_OK;
+}
+
+int ugks_sync(ugks_ctx *c)
+{
+    if (!c) return fail(c, UGKS_EINVAL, "%s", "NULL context");
+    return check_deferred(c, "ugks_sync");
+}
+
+int ugks_moments(ugks_ctx *c, double *W_stored, double *W_of_f, int on_dev)
+{
+    if (!c) return fail(c, UGKS_EINVAL, "%s", "NULL context");
+    if (!c->have_state) return fail(c, UGKS_ESTATE, "%s", "no state");
+    const UgksParams &P = c->P;
+    const cudaMemcpyKind kind = on_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (W_stored) CK(cudaMemcpyAsync(W_stored, P.W[c->cur], c->cells * 32, kind, c->st), "ugks_moments");
+    if (W_of_f) {
+        c->launches += launch_moments_of_f(P, P.f[c->cur], c->Wf_dev, c->st);
+        CK(cudaGetLastError(), "ugks_moments");
+        CK(cudaMemcpyAsync(W_of_f, c->Wf_dev, c->cells * 32, kind, c->st), "ugks_moments");
+    }
+    return check_deferred(c, "ugks_moments");
+}
+
+int ugks_get_f(ugks_ctx *c, double *f, int on_dev)
+{
+    if (!c || !f) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
+    if (!c->have_state) return fail(c, UGKS_ESTATE, "%s", "no state");
+    const UgksParams &P = c->P;
+    const cudaMemcpyKind kind = on_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    CK(cudaMemcpy2DAsync(f, (size_t)P.N * 8, P.f[c->cur], (size_t)P.Npad * 8, (size_t)P.N * 8, c->cells, kind, c->st), "ugks_get_f");
+    return check_deferred(c, "ugks_get_f");
+}
+
+int ugks_residual(ugks_ctx *c, double res[4])
+{
+    if (!c || !res) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
+    if (!c->have_res) return fail(c, UGKS_ESTATE, "%s", "ugks_residual before the first step");
+    c->launches += launch_residual_final(c->P, c->resblocks, c->res_dev, c->st);
+    CK(cudaGetLastError(), "ugks_residual");
+    CK(cudaMemcpyAsync(res, c->res_dev, 32, cudaMemcpyDeviceToHost, c->st), "ugks_residual");
+    return check_deferred(c, "ugks_residual");
+}
+
+}  // extern "C"

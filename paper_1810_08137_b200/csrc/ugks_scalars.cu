@@ -1,0 +1,353 @@
+// ugks_scalars.cu -- the O(faces) and O(cells) scalar stages: S2..S5 per face, wall density,
+// U1/U2 per cell (Eq. (4), Eq. (3) coefficients), the L2 residual (O11) and the setup of O0.
+// One thread per face / cell: these stages are "sequential" in the paper's wording; here they
+// run fully parallel ACROSS faces so that no CTA ever idles behind one face's scalar chain.
+#include "ugks_common.cuh"
+
+struct Prim { double rho, U, V, lam; };
+
+__device__ __forceinline__ Prim prim_of(const double W[4])
+{
+    Prim p;
+    p.rho = W[0];
+    const double ir = 1.0 / W[0];
+    p.U = W[1] * ir; p.V = W[2] * ir;
+    p.lam = W[0] / (2.0 * (W[3] - 0.5 * W[0] * (p.U * p.U + p.V * p.V)));
+    return p;
+}
+__device__ __forceinline__ double tau_of(const UgksParams &P, double rho, double lam)
+{
+    return 2.0 * P.mu_ref * pow(lam, 1.0 - P.omega) / rho;          // AMB-7
+}
+
+// <n^a t^b (c.psi)> for the normal-moment set X (full or half range) and tangential set Y
+__device__ __forceinline__ double mom_c(const double *X, const double *Y, const double c[4], int a, int b)
+{
+    return c[0] * X[a] * Y[b] + c[1] * X[a + 1] * Y[b] + c[2] * X[a] * Y[b + 1]
+         + 0.5 * c[3] * (X[a + 2] * Y[b] + X[a] * Y[b + 2]);
+}
+// out[r] += s * <n^a t^b psi_r (c.psi)>
+__device__ __forceinline__ void add_T(double out[4], double s, const double *X, const double *Y, const double c[4], int a, int b)
+{
+    out[0] += s * mom_c(X, Y, c, a, b);
+    out[1] += s * mom_c(X, Y, c, a + 1, b);
+    out[2] += s * mom_c(X, Y, c, a, b + 1);
+    out[3] += s * 0.5 * (mom_c(X, Y, c, a + 2, b) + mom_c(X, Y, c, a, b + 2));
+}
+// O6: c with rho <psi (c.psi)> = s  (K_int = 0)
+__device__ __forceinline__ void micro_slope(const Prim &p, const double s[4], double c[4])
+{
+    const double k = 2.0 * p.lam / p.rho, q2 = p.U * p.U + p.V * p.V, il = 1.0 / p.lam;
+    c[3] = k * p.lam * (2.0 * s[3] - 2.0 * p.U * s[1] - 2.0 * p.V * s[2] + s[0] * (q2 - il));
+    c[2] = k * (s[2] - p.V * s[0]) - p.V * c[3];
+    c[1] = k * (s[1] - p.U * s[0]) - p.U * c[3];
+    c[0] = s[0] / p.rho - p.U * c[1] - p.V * c[2] - 0.5 * (q2 + il) * c[3];
+}
+
+// W and tangential gradient of W (AMB-14) of the cell at `pos` on `line`, in the GLOBAL frame.
+// kind: 0 cell, 1 ghost, 2 wall(missing)
+template <int DIR>
+__device__ void cell_W_and_tgrad(const UgksParams &P, const double *W, int pos, int line, double Wc[4], double g[4], int *kind)
+{
+    const int n = DIR == 0 ? P.I : P.J, lo = DIR == 0 ? 0 : 2;
+    int side = -1;
+    if (pos < 0) { if (P.bc[lo] == BC_PERIODIC) pos += n; else side = lo; }
+    else if (pos >= n) { if (P.bc[lo + 1] == BC_PERIODIC) pos -= n; else side = lo + 1; }
+    for (int r = 0; r < 4; ++r) g[r] = 0.0;
+    if (side >= 0) {
+        if (P.bc[side] == BC_WALL) { *kind = 2; for (int r = 0; r < 4; ++r) Wc[r] = 0.0; return; }
+        *kind = 1;
+        for (int r = 0; r < 4; ++r) Wc[r] = P.Wb[side * 4 + r];
+        return;
+    }
+    *kind = 0;
+    const int i = DIR == 0 ? pos : line, j = DIR == 0 ? line : pos;
+    const double *w0 = W + ((size_t)j * P.I + i) * 4;
+    for (int r = 0; r < 4; ++r) Wc[r] = w0[r];
+    // tangential direction: y for x-faces, x for y-faces
+    const int nt = DIR == 0 ? P.J : P.I, tl = DIR == 0 ? 2 : 0;
+    const int tp = DIR == 0 ? j : i;
+    const double D = DIR == 0 ? P.dy : P.dx;
+    const double *wm = nullptr, *wp = nullptr;
+    int km = 0, kp = 0;                                              // 0 cell/ghost present, 2 wall
+    {
+        int t = tp - 1;
+        if (t < 0) { if (P.bc[tl] == BC_PERIODIC) t += nt; else if (P.bc[tl] == BC_FIXED) wm = P.Wb + tl * 4; else km = 2; }
+        if (!wm && !km) wm = W + (DIR == 0 ? ((size_t)t * P.I + i) : ((size_t)j * P.I + t)) * 4;
+        t = tp + 1;
+        if (t >= nt) { if (P.bc[tl + 1] == BC_PERIODIC) t -= nt; else if (P.bc[tl + 1] == BC_FIXED) wp = P.Wb + (tl + 1) * 4; else kp = 2; }
+        if (!wp && !kp) wp = W + (DIR == 0 ? ((size_t)t * P.I + i) : ((size_t)j * P.I + t)) * 4;
+    }
+    for (int r = 0; r < 4; ++r) {
+        if (!km && !kp) g[r] = (wp[r] - wm[r]) / (2.0 * D);
+        else if (km && !kp) g[r] = (wp[r] - w0[r]) / D;
+        else if (kp && !km) g[r] = (w0[r] - wm[r]) / D;
+    }
+}
+
+__device__ __forceinline__ void swap12(double w[4]) { const double t = w[1]; w[1] = w[2]; w[2] = t; }
+
+template <int DIR>
+__device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
+{
+    const size_t face = DIR == 0 ? (size_t)line * (P.I + 1) + pos : (size_t)pos * P.I + line;
+    double M[11];
+    for (int v = 0; v < 11; ++v) M[v] = 0.0;
+    const double *mp = P.mom[DIR] + face * P.nchunk * NMOM;
+    for (int c = 0; c < P.nchunk; ++c)
+        for (int v = 0; v < 11; ++v) M[v] += mp[c * NMOM + v];
+    double *cf = P.coef[DIR] + face * NCOEF, *fw = P.fw[DIR] + face * 4;
+    const double h = 0.5 * (DIR == 0 ? P.dx : P.dy), ell = DIR == 0 ? P.dy : P.dx, dt = P.dt;
+
+    double WL[4], WR[4], gL[4], gR[4];
+    int kL, kR;
+    cell_W_and_tgrad<DIR>(P, P.W[cur], pos - 1, line, WL, gL, &kL);
+    cell_W_and_tgrad<DIR>(P, P.W[cur], pos, line, WR, gR, &kR);
+
+    if (kL == 2 || kR == 2) {                                        // O9: diffuse wall
+        const int side = (DIR == 0 ? 0 : 2) + (kR == 2 ? 1 : 0);
+        const double *G = P.wallG + side * 4;
+        const double S[4] = { M[1], M[4], M[5], M[6] };              // sum_{incoming} w n psi_loc f_face
+        const double rho_w = -S[0] / G[0];
+        double F[4];
+        F[0] = 0.0;                                                  // S0 + rho_w G0 = 0 by definition of rho_w
+        for (int r = 1; r < 4; ++r) F[r] = ell * dt * (S[r] + rho_w * G[r]);
+        if (DIR == 1) swap12(F);
+        for (int r = 0; r < 4; ++r) fw[r] = F[r];
+        for (int r = 0; r < NCOEF; ++r) cf[r] = 0.0;
+        cf[CF_MT4] = dt;                                             // F_q = ell n dt f_w through the common formula
+        cf[CF_TYPE] = 1.0; cf[CF_RHOW] = rho_w;
+        return;
+    }
+    if (DIR == 1) { swap12(WL); swap12(WR); swap12(gL); swap12(gR); }
+
+    // S1: interface state
+    double W0[4] = { M[0], M[1], M[2], M[3] };
+    const Prim p0 = prim_of(W0);
+    if (!(p0.rho > 0.0) || !(p0.lam > 0.0)) atomicOr(P.status, 1);
+    // S2: Maxwellian moments (O4)
+    double XL[7], XR[7], XF[7], Y[7];
+    {
+        const double sl = sqrt(p0.lam), e = 0.5 * exp(-p0.lam * p0.U * p0.U) / sqrt(UGKS_PI * p0.lam);
+        const double il2 = 0.5 / p0.lam;
+        XL[0] = 0.5 * erfc(-sl * p0.U); XL[1] = p0.U * XL[0] + e;
+        XR[0] = 0.5 * erfc(sl * p0.U);  XR[1] = p0.U * XR[0] - e;
+        Y[0] = 1.0; Y[1] = p0.V;
+        for (int q = 0; q < 5; ++q) {
+            XL[q + 2] = p0.U * XL[q + 1] + (q + 1) * il2 * XL[q];
+            XR[q + 2] = p0.U * XR[q + 1] + (q + 1) * il2 * XR[q];
+            Y[q + 2] = p0.V * Y[q + 1] + (q + 1) * il2 * Y[q];
+        }
+        for (int q = 0; q < 7; ++q) XF[q] = XL[q] + XR[q];
+    }
+    // S3: tau and the time integrals (O5, AMB-11)
+    const double tau = tau_of(P, p0.rho, p0.lam), x = dt / tau;
+    double Mt1, Mt2, Mt3, Mt4, Mt5;
+    if (x >= 1e-3) {
+        const double em = -expm1(-x), E = 1.0 - em;
+        Mt4 = tau * em; Mt5 = tau * (Mt4 - dt * E); Mt1 = dt - Mt4;
+        Mt2 = -tau * Mt1 + Mt5; Mt3 = 0.5 * dt * dt - tau * Mt1;
+    } else {
+        const double d2 = dt * dt;
+        Mt4 = dt * (1.0 + x * (-1.0 / 2 + x * (1.0 / 6 + x * (-1.0 / 24 + x * (1.0 / 120)))));
+        Mt1 = dt * x * (1.0 / 2 + x * (-1.0 / 6 + x * (1.0 / 24 + x * (-1.0 / 120))));
+        Mt5 = d2 * (0.5 + x * (-1.0 / 3 + x * (1.0 / 8 + x * (-1.0 / 30 + x * (1.0 / 144)))));
+        Mt3 = d2 * x * (1.0 / 6 + x * (-1.0 / 24 + x * (1.0 / 120 + x * (-1.0 / 720))));
+        Mt2 = d2 * x * (-1.0 / 6 + x * (1.0 / 12 + x * (-1.0 / 40 + x * (1.0 / 180))));
+    }
+    // S4: micro-slopes (O6)
+    double sL[4], sR[4], sb[4], aL[4], aR[4], bb[4], A[4];
+    for (int r = 0; r < 4; ++r) {
+        sL[r] = (W0[r] - WL[r]) / h;
+        sR[r] = (WR[r] - W0[r]) / h;
+        sb[r] = 0.5 * (gL[r] + gR[r]);
+    }
+    micro_slope(p0, sL, aL); micro_slope(p0, sR, aR); micro_slope(p0, sb, bb);
+    double sA[4] = { 0, 0, 0, 0 };
+    add_T(sA, -p0.rho, XL, Y, aL, 1, 0);
+    add_T(sA, -p0.rho, XR, Y, aR, 1, 0);
+    add_T(sA, -p0.rho, XF, Y, bb, 0, 1);
+    micro_slope(p0, sA, A);
+    // S5: hydrodynamic flux (O7) + the free-transport sums of S7 (O8)
+    double F[4];
+    F[0] = p0.rho * Mt1 * XF[1];
+    F[1] = p0.rho * Mt1 * XF[2];
+    F[2] = p0.rho * Mt1 * XF[1] * Y[1];
+    F[3] = p0.rho * Mt1 * 0.5 * (XF[3] + XF[1] * Y[2]);
+    add_T(F, p0.rho * Mt2, XL, Y, aL, 2, 0);
+    add_T(F, p0.rho * Mt2, XR, Y, aR, 2, 0);
+    add_T(F, p0.rho * Mt2, XF, Y, bb, 1, 1);
+    add_T(F, p0.rho * Mt3, XF, Y, A, 1, 0);
+    F[0] += Mt4 * M[1] - Mt5 * M[7];
+    F[1] += Mt4 * M[4] - Mt5 * M[8];
+    F[2] += Mt4 * M[5] - Mt5 * M[9];
+    F[3] += Mt4 * M[6] - Mt5 * M[10];
+    for (int r = 0; r < 4; ++r) F[r] *= ell;
+    if (DIR == 1) swap12(F);
+    for (int r = 0; r < 4; ++r) fw[r] = F[r];
+
+    cf[CF_C0] = p0.rho * p0.lam / UGKS_PI; cf[CF_U] = p0.U; cf[CF_V] = p0.V; cf[CF_LAM] = p0.lam;
+    cf[CF_MT1] = Mt1; cf[CF_MT2] = Mt2; cf[CF_MT3] = Mt3; cf[CF_MT4] = Mt4; cf[CF_MT5] = Mt5;
+    for (int r = 0; r < 4; ++r) { cf[CF_AL + r] = aL[r]; cf[CF_AR + r] = aR[r]; cf[CF_B + r] = bb[r]; cf[CF_A + r] = A[r]; }
+    cf[CF_TYPE] = 0.0; cf[CF_RHOW] = 0.0; cf[27] = tau;
+}
+
+__global__ void __launch_bounds__(128) k_face_scalars(const UgksParams P, const int cur)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nfx = nfaces_x(P), nfy = nfaces_y(P);
+    if (t < nfx) face_scalars<0>(P, cur, t % (P.I + 1), t / (P.I + 1));
+    else if (t < nfx + nfy) { const int s = t - nfx; face_scalars<1>(P, cur, s / P.I, s % P.I); }
+}
+
+// U1 + U2 per cell, plus the partial sums of the residual (O11)
+__global__ void __launch_bounds__(128) k_cell_scalars(const UgksParams P, const int cur)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int ncell = P.I * P.J;
+    double part[8] = { 0, 0, 0, 0, 0, 0, 0, 0 };
+    if (c < ncell) {
+        const int i = c % P.I, j = c / P.I;
+        const double *Wn = P.W[cur] + (size_t)c * 4;
+        const double *fxm = P.fw[0] + ((size_t)j * (P.I + 1) + i) * 4, *fxp = fxm + 4;
+        const double *fym = P.fw[1] + ((size_t)j * P.I + i) * 4, *fyp = fym + (size_t)P.I * 4;
+        const double iOm = 1.0 / (P.dx * P.dy);
+        double Wp[4], Wo[4];
+        for (int r = 0; r < 4; ++r) {
+            Wo[r] = Wn[r];
+            Wp[r] = Wo[r] + (((fxm[r] - fxp[r]) + fym[r]) - fyp[r]) * iOm;   // P:L45 Eq. (4)
+            P.W[cur ^ 1][(size_t)c * 4 + r] = Wp[r];
+            const double d = Wp[r] - Wo[r];
+            part[r] = d * d; part[4 + r] = fabs(Wp[r]);
+        }
+        const Prim pn = prim_of(Wo), pp = prim_of(Wp);
+        if (!(pp.rho > 0.0) || !(pp.lam > 0.0)) atomicOr(P.status, 2);
+        const double tn = tau_of(P, pn.rho, pn.lam), tp = tau_of(P, pp.rho, pp.lam);
+        const double inv = 1.0 / (1.0 + 0.5 * P.dt / tp);
+        double *cc = P.cellc + (size_t)c * NCELL;
+        cc[CC_GN] = pn.rho * pn.lam / UGKS_PI * (0.5 * P.dt / tn) * inv; cc[CC_UN] = pn.U; cc[CC_VN] = pn.V; cc[CC_LN] = pn.lam;
+        cc[CC_GP] = pp.rho * pp.lam / UGKS_PI * (0.5 * P.dt / tp) * inv; cc[CC_UP] = pp.U; cc[CC_VP] = pp.V; cc[CC_LP] = pp.lam;
+        cc[CC_KF] = (1.0 - 0.5 * P.dt / tn) * inv;
+        cc[CC_KD] = iOm * inv;
+    }
+    __shared__ double sh[4][8];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int v = 0; v < 8; ++v) {
+        const double s = warp_sum(part[v]);
+        if (lane == 0) sh[warp][v] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        double s = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) s += sh[w][threadIdx.x];
+        P.respart[(size_t)blockIdx.x * 8 + threadIdx.x] = s;
+    }
+}
+
+// O11: fixed-order final sum of the per-block partials (deterministic, no fp64 atomics)
+__global__ void __launch_bounds__(256) k_residual_final(const double *part, int nblocks, double ncell, double *res)
+{
+    __shared__ double sh[8][8];
+    const int v = threadIdx.x & 7, g = threadIdx.x >> 3;            // 32 groups of 8
+    double s = 0.0;
+    for (int b = g; b < nblocks; b += 32) s += part[(size_t)b * 8 + v];
+    // reduce over the 32 groups: lanes with equal v are 8 apart inside a warp (4 groups per warp)
+    s += __shfl_xor_sync(0xffffffffu, s, 8);
+    s += __shfl_xor_sync(0xffffffffu, s, 16);
+    if ((threadIdx.x & 31) < 8) sh[threadIdx.x >> 5][v] = s;
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += sh[w][threadIdx.x];
+        sh[0][threadIdx.x] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) res[threadIdx.x] = sqrt(ncell * sh[0][threadIdx.x]) / (sh[0][4 + threadIdx.x] + 1e-300);
+}
+
+// O0: ghost rows, wall Maxwellians, W_b and the outgoing wall sums G (one block per side)
+__global__ void __launch_bounds__(256) k_setup(const UgksParams P, const double *bcprim, double *ghost, double *wallg,
+                                               double *Wb, double *wallG)
+{
+    const int side = blockIdx.x, type = P.bc[side];
+    const double rho = type == BC_FIXED ? bcprim[side * 4 + 0] : 1.0, U = bcprim[side * 4 + 1], V = bcprim[side * 4 + 2];
+    const double lam = 1.0 / bcprim[side * 4 + 3];
+    const int dir = side >> 1;
+    const double sgn = (side & 1) ? 1.0 : -1.0;                      // outward normal = sgn * e_dir
+    double g[4] = { 0, 0, 0, 0 };
+    for (int q = threadIdx.x; q < P.Npad; q += blockDim.x) {
+        double val = 0.0;
+        if (q < P.N && type != BC_PERIODIC) {
+            const int k = q % P.Nu, m = q / P.Nu;
+            const double u = P.u[k], v = P.v[m], du = u - U, dv = v - V;
+            val = rho * (lam / UGKS_PI) * exp(-lam * (du * du + dv * dv));
+            if (type == BC_WALL) {
+                const double n = dir == 0 ? u : v, t = dir == 0 ? v : u, w = P.wu[k] * P.wv[m];
+                if (sgn * n < 0.0) {                                 // leaves the wall (1-H)
+                    const double wn = w * n * val;
+                    g[0] += wn; g[1] += wn * n; g[2] += wn * t; g[3] += wn * 0.5 * (n * n + t * t);
+                }
+            }
+        }
+        ghost[(size_t)side * P.Npad + q] = type == BC_FIXED ? val : 0.0;
+        wallg[(size_t)side * P.Npad + q] = type == BC_WALL ? val : 0.0;
+    }
+    __shared__ double sh[8][4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int r = 0; r < 4; ++r) { const double s = warp_sum(g[r]); if (lane == 0) sh[warp][r] = s; }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += sh[w][threadIdx.x];
+        wallG[side * 4 + threadIdx.x] = s;
+    }
+    if (threadIdx.x == 0) {
+        Wb[side * 4 + 0] = rho; Wb[side * 4 + 1] = rho * U; Wb[side * 4 + 2] = rho * V;
+        Wb[side * 4 + 3] = 0.5 * rho * (U * U + V * V) + rho / (2.0 * lam);
+    }
+}
+
+// O12: W_of_f[c] = sum_q w_q psi_q f[c][q]; one warp per cell
+__global__ void __launch_bounds__(256) k_moments_of_f(const UgksParams P, const double *f, double *Wf)
+{
+    const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (c >= P.I * P.J) return;
+    const double *row = f + (size_t)c * P.Npad;
+    double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+    for (int q = lane; q < P.N; q += 32) {
+        const int k = q % P.Nu, m = q / P.Nu;
+        const double u = P.u[k], v = P.v[m], wf = P.wu[k] * P.wv[m] * row[q];
+        s0 += wf; s1 = fma(wf, u, s1); s2 = fma(wf, v, s2); s3 = fma(wf, 0.5 * (u * u + v * v), s3);
+    }
+    s0 = warp_sum(s0); s1 = warp_sum(s1); s2 = warp_sum(s2); s3 = warp_sum(s3);
+    if (lane == 0) { double *o = Wf + (size_t)c * 4; o[0] = s0; o[1] = s1; o[2] = s2; o[3] = s3; }
+}
+
+int launch_face_scalars(const UgksParams &P, int cur, cudaStream_t st)
+{
+    const int n = nfaces_x(P) + nfaces_y(P);
+    k_face_scalars<<<(n + 127) / 128, 128, 0, st>>>(P, cur);
+    return 1;
+}
+int launch_cell_scalars(const UgksParams &P, int cur, int resblocks, cudaStream_t st)
+{
+    k_cell_scalars<<<resblocks, 128, 0, st>>>(P, cur);
+    return 1;
+}
+int launch_residual_final(const UgksParams &P, int resblocks, double *res_dev, cudaStream_t st)
+{
+    k_residual_final<<<1, 256, 0, st>>>(P.respart, resblocks, (double)P.I * P.J, res_dev);
+    return 1;
+}
+int launch_setup(const UgksParams &P, const double *bc_prims, double *ghost, double *wallg, double *Wb, double *wallG,
+                 cudaStream_t st)
+{
+    k_setup<<<4, 256, 0, st>>>(P, bc_prims, ghost, wallg, Wb, wallG);
+    return 1;
+}
+int launch_moments_of_f(const UgksParams &P, const double *f, double *Wf, cudaStream_t st)
+{
+    const int ncell = P.I * P.J;
+    k_moments_of_f<<<(ncell + 7) / 8, 256, 0, st>>>(P, f, Wf);
+    return 1;
+}

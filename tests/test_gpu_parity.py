@@ -1,0 +1,143 @@
+"""GPU-vs-oracle parity (T2/T3 of DESIGN.md): the CUDA path through the C ABI against the CPU oracle on the
+same seeded inputs, element by element.  Tolerances are north_star's: <= 1e-12 after 1 step, <= 1e-10 after
+100 steps, in the metrics of AMB-17 (tests/util.py)."""
+import numpy as np
+import pytest
+
+import workloads
+from tests.util import err_f, err_W
+
+pytestmark = pytest.mark.gpu
+
+TOL_1 = 1e-12
+TOL_100 = 1e-10
+
+
+def _run_pair(p, steps, W=None, f=None, threads=8):
+    from oracle import Oracle
+    from paper_1810_08137_b200 import Ugks
+    if W is None:
+        W, f, _ = workloads.initial_state(p)
+    o = Oracle(p, threads=threads)
+    o.set_state(W, f)
+    g = Ugks(p)
+    assert abs(g.dt - o.dt) <= 1e-16 * o.dt and abs(g.mu_ref - o.mu_ref) <= 1e-16 * o.mu_ref
+    g.set_state(W, f)
+    o.step(steps)
+    g.step(steps)
+    out = dict(ef=err_f(g.f(), o.f()), eW=err_W(g.W(), o.W()), res_g=g.residual(), res_o=o.residual(),
+               Wf_g=g.W_of_f(), Wf_o=o.W_of_f(), g=g, o=o)
+    return out
+
+
+def _check(r, tol):
+    assert r["ef"] <= tol, r["ef"]
+    assert r["eW"] <= tol, r["eW"]
+    assert np.allclose(r["res_g"], r["res_o"], rtol=1e-7, atol=1e-18)
+    assert err_W(r["Wf_g"], r["Wf_o"]) <= tol
+
+
+@pytest.mark.parametrize("steps,tol", [(1, TOL_1), (10, TOL_100)])
+def test_C1_channel(steps, tol):
+    _check(_run_pair(workloads.channel_config("C1"), steps), tol)
+
+
+def test_C2_channel_reduced_100_steps():
+    """C2's velocity grid and physics on a 48x20 mesh (several strips + ragged tail), 100 steps."""
+    _check(_run_pair(workloads.channel_config("C2", I=48, J=20), 100), TOL_100)
+
+
+@pytest.mark.parametrize("name,I,J", [("C3", 40, 12), ("C4", 37, 9), ("C5", 6, 5)])
+def test_config_velocity_grids_one_step(name, I, J):
+    """Each config's velocity grid (28x28, 40x40 two chunks, 200x200 fifty chunks) on a small ragged mesh."""
+    _check(_run_pair(workloads.channel_config(name, I=I, J=J), 1), TOL_1)
+
+
+@pytest.mark.parametrize("nu,nv", [(29, 29), (13, 9), (7, 33), (16, 12)])
+def test_periodic_box_odd_grids(nu, nv):
+    """Odd grids contain u = 0 / v = 0 nodes (H(0) = 1/2, AMB-5) and rows that are not 16-byte multiples."""
+    p = workloads.periodic_box(9, 7, nu, nv, a=5.0, Kn=0.05, seed=5, bu=6.0, lx=1.3, ly=0.7)
+    _check(_run_pair(p, 3), 3 * TOL_1)
+
+
+def test_closed_box_walls_on_all_sides():
+    u, wu = workloads.trapezoid_grid(17, 6.0)
+    wall = (workloads.BC_WALL, 1.0, 0.1, -0.05, 1.2)
+    p = workloads.Problem(I=6, J=5, x0=0.0, x1=1.0, y0=0.0, y1=1.0, u=u, wu=wu, v=u.copy(), wv=wu.copy(), Kn=0.1,
+                          bcs=[wall] * 4, cfl=0.8, seed=9, eps=(0.05, 0.05, 0.05, 0.05), rho_drop=0.0)
+    r = _run_pair(p, 4)
+    _check(r, 4 * TOL_1)
+    W0, _, _ = workloads.initial_state(p)
+    assert abs(r["g"].W()[..., 0].sum() - W0[..., 0].sum()) < 1e-13 * W0[..., 0].sum()      # P11 on the GPU
+
+
+def test_fixed_sides_in_y_and_walls_in_x():
+    p = workloads.channel_config("C1", I=7, J=11, Nuv=14)
+    p.bcs = [p.bcs[2], p.bcs[3], (workloads.BC_FIXED, 1.0, 0.0, 0.05, 1.0), (workloads.BC_FIXED, 0.9, 0.0, 0.0, 1.1)]
+    _check(_run_pair(p, 3), 3 * TOL_1)
+
+
+def test_rough_data_limiter_active_and_stiff_and_collisionless():
+    rng = np.random.default_rng(3)
+    for kn in (1e-5, 0.1, 1e9):
+        p = workloads.periodic_box(8, 6, 16, 16, a=6.0, Kn=kn, seed=4)
+        W, f, _ = workloads.initial_state(p)
+        f = f * rng.uniform(0.5, 1.5, f.shape)
+        _check(_run_pair(p, 2, W, f), 2 * TOL_1)
+
+
+def test_gpu_fixed_point_and_conservation():
+    """P6/P7 directly on the GPU path."""
+    from paper_1810_08137_b200 import Ugks
+    p = workloads.periodic_box(8, 6, 16, 20, a=6.0, Kn=0.1, seed=3)
+    W, f, _ = workloads.initial_state(p)
+    g = Ugks(p)
+    g.set_state(W, f)
+    g.step(5)
+    tot0, tot = W.reshape(-1, 4).sum(0), g.W().reshape(-1, 4).sum(0)
+    assert np.all(np.abs(tot - tot0) < 1e-13 * tot0[0])
+    ones = np.ones((p.J, p.I))
+    f = workloads.maxwellian_field(p, 0.9 * ones, 0.3 * ones, -0.1 * ones, ones / 1.2)
+    lam = 1.2
+    W = np.broadcast_to(np.array([0.9, 0.27, -0.09, 0.5 * 0.9 * 0.1 + 0.9 / (2 * lam)]), (p.J, p.I, 4)).copy()
+    g.set_state(W, f)
+    g.step(3)
+    assert np.max(np.abs(g.W() - W)) < 1e-15 and err_f(g.f(), f) < 1e-15
+
+
+def test_bit_reproducible_run_to_run():
+    from paper_1810_08137_b200 import Ugks
+    p = workloads.channel_config("C1")
+    W, f, _ = workloads.initial_state(p)
+    outs = []
+    for _ in range(2):
+        g = Ugks(p)
+        g.set_state(W, f)
+        g.step(5)
+        outs.append((g.f(), g.W()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+def test_device_pointers_and_errors():
+    import torch
+    from paper_1810_08137_b200 import Ugks, UgksError
+    p = workloads.channel_config("C1")
+    W, f, _ = workloads.initial_state(p)
+    g = Ugks(p)
+    with pytest.raises(UgksError):
+        g.step(1)                                           # UGKS_ESTATE: no state yet
+    Wd, fd = torch.from_numpy(W).cuda(), torch.from_numpy(f).cuda()
+    g.set_state(Wd, fd)
+    g.step(2)
+    fo = torch.empty_like(fd)
+    g.f(out=fo)
+    h = Ugks(p)
+    h.set_state(W, f)
+    h.step(2)
+    assert np.array_equal(fo.cpu().numpy(), h.f())
+    # a non-physical state is reported at the next synchronising call
+    bad = W.copy(); bad[..., 3] = -1.0
+    g.set_state(bad, f)
+    g.step(1)
+    with pytest.raises(UgksError):
+        g.sync()

@@ -1,0 +1,297 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the B200 UGKS step (fp64 cell x velocity-point updates/s) and its roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference] [--no-extra]
+
+A "step" is one pass of the whole hot path (face moments x/y, face scalars, cell scalars, flux+update) over the
+synthetic channel workload.  N > 1 (under torchrun) runs N independent replicas ("replicas only": the path is
+single-GPU by north_star); value = points all ranks processed / max-over-ranks device time.
+Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle on a bounded sample instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import psutil
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "fp64 UGKS cell x velocity-point updates/s"
+UNIT = "updates/s"
+ALG_BYTES_PER_POINT = 16.0          # read f^n once, write f^{n+1} once
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+            except Exception:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def dist_setup(n_gpus, backend=None):
+    """(rank, world, dist or None).  One process per GPU under torchrun; plain python for N = 1."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world == 1:
+        return 0, 1, None
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    if not dist.is_initialized():
+        dist.init_process_group(backend=backend or "nccl")
+    return rank, world, dist
+
+
+def dist_max(dist, value, device="cpu"):
+    """max over ranks of a python float (identity for a single process)."""
+    if dist is None:
+        return value
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def dist_sum(dist, value, device="cpu"):
+    if dist is None:
+        return value
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def oracle_sample(p, seconds_hint=15.0):
+    """The CPU oracle as it stands on a bounded sample of workload p: same physics and velocity grid, the mesh
+    cut to the first rows (J_s rows of I cells, walls kept), enough steps for ~10-30 s of CPU work."""
+    from oracle import Oracle
+    cores = os.cpu_count() or 1
+    est = 4.0e6 * cores * 0.7                                   # updates/s guess, only to size the sample
+    pts_target = est * seconds_hint / 3.0
+    Js = int(max(4, min(p.J, pts_target / (p.I * p.N))))
+    ps = workloads.channel_config(p.name, I=p.I, J=Js)
+    W, f, _ = workloads.initial_state(ps)
+    o = Oracle(ps, threads=cores)
+    o.set_state(W, f)
+    o.step(1)                                                   # warm caches / page in
+    t0 = time.perf_counter()
+    nst = 0
+    while True:
+        o.step(1); nst += 1
+        el = time.perf_counter() - t0
+        if el > seconds_hint * 0.6 or nst >= 50:
+            break
+    return ps.points * nst / el, cores, f"{p.name} physics and {p.Nu}x{p.Nv} velocity grid on a {ps.I}x{ps.J} mesh, {nst} steps, {cores} OpenMP threads", el / nst
+
+
+def run_reference(args):
+    rank, world, dist = dist_setup(args.gpus, backend="gloo")
+    if rank != 0:
+        return
+    p = workloads.channel_config(args.config)
+    steps = max(1, args.steps)
+    from oracle import Oracle
+    cores = os.cpu_count() or 1
+    Js = int(max(4, min(p.J, 2.5e7 / (p.I * p.N))))
+    ps = workloads.channel_config(p.name, I=p.I, J=Js)
+    W, f, _ = workloads.initial_state(ps)
+    o = Oracle(ps, threads=cores)
+    o.set_state(W, f)
+    for _ in range(max(1, args.warmup)):
+        o.step(1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(1)
+    el = time.perf_counter() - t0
+    val = ps.points * steps / el
+    sample = f"{p.name} physics and {p.Nu}x{p.Nv} velocity grid on a {ps.I}x{ps.J} mesh per step, {cores} OpenMP threads"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * el / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": _workload_name(p), "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def _workload_name(p):
+    return f"{p.name}: channel {p.I}x{p.J} cells, {p.Nu}x{p.Nv} velocity grid, Kn={p.Kn}"
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C3", choices=list(workloads.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extra", action="store_true", help="skip the other configs / cpu baseline (N=1 default runs them)")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_1810_08137_b200 import Ugks
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the UGKS path has no CPU fallback")
+    rank, world, dist = dist_setup(args.gpus)
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dev = f"cuda:{local}"
+    torch.cuda.set_device(local)
+    warmup = max(3, args.warmup)
+    steps = max(1, args.steps)
+    peak, peak_src = _peaks()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def measure(p, steps, warmup, e2e, kernels):
+        fh = torch.empty((p.J, p.I, p.Nv, p.Nu), dtype=torch.float64, pin_memory=True)
+        W, _, _ = workloads.initial_state(p, out_f=fh.numpy())          # f is drawn straight into pinned memory
+        Wh = torch.from_numpy(W).pin_memory()
+        del W
+        g = Ugks(p, device=dev)
+        g.set_state(Wh.to(dev), fh.to(dev))
+        torch.cuda.empty_cache()
+        g.step(warmup); g.sync()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        l0 = g.launch_count
+        with ClockSampler(local) as cs:
+            e0.record()
+            g.step(steps)
+            e1.record()
+            barrier()
+        ms = dist_max(dist, e0.elapsed_time(e1), dev)
+        res = {"ms": ms, "launches": g.launch_count - l0, "clocks": cs.summary(), "points": p.points}
+        if kernels:
+            g.set_option("profile", 1)
+            g.step(steps)
+            kt = g.kernel_times()
+            g.set_option("profile", 0)
+            res["kernels"] = {k: {"ms_per_launch": t / max(n, 1), "launches": n} for k, (t, n) in kt.items()}
+        if e2e:
+            Wo = torch.empty_like(Wh).pin_memory()
+            fo = torch.empty_like(fh).pin_memory()
+            reps = 3
+            for it in range(reps + 1):                       # first pass untimed (page-locks, first-touch)
+                if it == 1:
+                    barrier(); t0 = time.perf_counter()
+                g.set_state(Wh.numpy(), fh.numpy())          # host -> device inside the timed region
+                g.step(1)
+                g.f(out=fo.numpy()); g.W(out=Wo.numpy())     # device -> host
+            barrier()
+            el = dist_max(dist, time.perf_counter() - t0, dev)
+            res["e2e"] = {"value": world * p.points * reps / el, "unit": UNIT,
+                          "h2d_bytes_per_step": int(fh.numel() * 8 + Wh.numel() * 8),
+                          "d2h_bytes_per_step": int(fo.numel() * 8 + Wo.numel() * 8), "ms_per_step": 1e3 * el / reps}
+        g.close()
+        del g, Wh, fh
+        torch.cuda.empty_cache()
+        return res
+
+    p = workloads.channel_config(args.config)
+    r = measure(p, steps, warmup, e2e=not args.no_e2e, kernels=True)
+    value = world * p.points * steps / (r["ms"] * 1e-3)
+    dom = max(r["kernels"], key=lambda k: r["kernels"][k]["ms_per_launch"])
+    share = {k: v["ms_per_launch"] for k, v in r["kernels"].items()}
+    tot = sum(share.values())
+    # bytes the dominant kernel must move per launch: flux_update reads f once and writes f once (16 B/pt);
+    # a face_moments launch reads f once (8 B/pt).  DESIGN.md "Roofline".
+    dom_bytes = (16.0 if dom == "flux_update" else 8.0) * p.points
+    achieved = dom_bytes / (r["kernels"][dom]["ms_per_launch"] * 1e-3) / 1e9
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": r["ms"] / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": _workload_name(p), "points_per_step": p.points, "parallelism": f"replicas x{world}",
+                       "l2": "inputs larger than L2 (one copy of f = %.0f MB), no flush" % (p.points * 8 / 1e6)
+                       if p.points * 8 > 126e6 else "L2-resident workload (f = %.0f MB), no flush" % (p.points * 8 / 1e6)},
+            "clocks": r["clocks"], "gpu_launches": r["launches"],
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "kernel_share_of_step": share[dom] / tot,
+                         "kernel_ms": {k: round(v, 5) for k, v in share.items()},
+                         "step_frac_of_16B_floor": ALG_BYTES_PER_POINT * value / world / 1e9 / peak},
+            "e2e": r.get("e2e")}
+    if rank == 0 and world == 1 and not args.no_extra:
+        v, cores, sample, _ = oracle_sample(p)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        others = {}
+        for name in workloads.CONFIGS:
+            if name == args.config or name == "C1":
+                continue
+            q = workloads.channel_config(name)
+            if q.points * 8 * 2.2 > psutil.virtual_memory().available:
+                others[name] = {"skipped": "host RAM too small to stage the input"}
+                continue
+            st = {"C2": 50, "C3": 10, "C4": 4, "C5": 6}[name]
+            rr = measure(q, st, 3, e2e=False, kernels=True)
+            others[name] = {"value": q.points * st / (rr["ms"] * 1e-3), "ms_per_step": rr["ms"] / st, "steps": st,
+                            "workload": _workload_name(q),
+                            "kernel_ms": {k: round(v["ms_per_launch"], 5) for k, v in rr["kernels"].items()},
+                            "step_frac_of_16B_floor": ALG_BYTES_PER_POINT * q.points * st / (rr["ms"] * 1e-3) / 1e9 / peak}
+        line["other_workloads"] = others
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -89,8 +89,14 @@ double ugks_mu_ref(const ugks_ctx *);
 long ugks_step_count(const ugks_ctx *);
 /* Kernels launched by this context since ugks_init (for bench.py's gpu_launches). */
 long ugks_launch_count(const ugks_ctx *);
-/* Tuning knobs, for experiments: name in {"strip", "chunk_m", "graph"}; returns UGKS_EINVAL for unknown names. */
+/* Tuning knobs: name in {"strip" (faces/cells per CTA march), "chunk_m" (velocity rows per chunk), "R" (velocity
+ * rows processed in parallel by a CTA), "profile" (1: time every kernel of ugks_step with CUDA events)}.
+ * UGKS_EINVAL for unknown names or values that do not fit shared memory / the allocated buffers. */
 int ugks_set_option(ugks_ctx *, const char *name, int value);
+/* With option "profile" on: accumulated device time in ms and launch counts of the five kernels of a step since
+ * the last call, in launch order: face_moments(x), face_moments(y), face_scalars, cell_scalars, flux_update.
+ * Synchronises the stream and resets the accumulators. */
+int ugks_kernel_times(ugks_ctx *, double ms[5], long counts[5]);
 const char *ugks_last_error(const ugks_ctx *);           /* library-owned string; ctx may be NULL */
 const char *ugks_version(void);
 void ugks_destroy(ugks_ctx *);

@@ -13,7 +13,7 @@ _dp = C.POINTER(C.c_double)
 
 EXPORTS = ["ugks_workspace_bytes", "ugks_init", "ugks_set_state", "ugks_step", "ugks_moments", "ugks_get_f",
            "ugks_residual", "ugks_sync", "ugks_dt", "ugks_mu_ref", "ugks_step_count", "ugks_launch_count",
-           "ugks_set_option", "ugks_last_error", "ugks_version", "ugks_destroy"]
+           "ugks_set_option", "ugks_kernel_times", "ugks_last_error", "ugks_version", "ugks_destroy"]
 
 
 class UgksError(RuntimeError):
@@ -70,6 +70,7 @@ def lib():
         L.ugks_step_count.argtypes = [vp]; L.ugks_step_count.restype = C.c_long
         L.ugks_launch_count.argtypes = [vp]; L.ugks_launch_count.restype = C.c_long
         L.ugks_set_option.argtypes = [vp, C.c_char_p, C.c_int]
+        L.ugks_kernel_times.argtypes = [vp, _dp, C.POINTER(C.c_long)]
         L.ugks_last_error.argtypes = [vp]; L.ugks_last_error.restype = C.c_char_p
         L.ugks_version.argtypes = []; L.ugks_version.restype = C.c_char_p
         L.ugks_destroy.argtypes = [vp]; L.ugks_destroy.restype = None
@@ -158,6 +159,15 @@ class Ugks:
 
     def set_option(self, name, value):
         self._chk(lib().ugks_set_option(self._h, name.encode(), int(value)))
+
+    KERNELS = ("face_moments_x", "face_moments_y", "face_scalars", "cell_scalars", "flux_update")
+
+    def kernel_times(self):
+        """{kernel: (total ms, launches)} since the last call (needs set_option("profile", 1))."""
+        ms = np.zeros(5)
+        cnt = (C.c_long * 5)()
+        self._chk(lib().ugks_kernel_times(self._h, ms.ctypes.data_as(_dp), cnt))
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(self.KERNELS)}
 
     def set_state(self, W, f):
         pw, dw = self._ptr(W, self.I * self.J * 4)

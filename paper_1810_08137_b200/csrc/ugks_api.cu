@@ -17,6 +17,9 @@ struct ugks_ctx {
     double *res_dev, *bcprim_dev, *Wf_dev;
     double *ghost, *wallg, *Wb, *wallG;     // non-const aliases of the P fields
     size_t cells;
+    int profile;              // option "profile": time every kernel of ugks_step with CUDA events
+    cudaEvent_t *ev; int nev, nev_used;
+    double kms[5]; long kcnt[5];
     char err[256];
 };
 
@@ -188,6 +191,8 @@ void ugks_destroy(ugks_ctx *c)
 {
     if (!c) return;
     cudaStreamSynchronize(c->st);
+    for (int i = 0; i < c->nev; ++i) cudaEventDestroy(c->ev[i]);
+    free(c->ev);
     free(c);
 }
 
@@ -218,6 +223,7 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
         if (setup_moments_attributes(P) || setup_update_attributes(P)) return cuda_fail(c, cudaGetLastError(), "ugks_set_option");
         return UGKS_OK;
     }
+    if (!strcmp(name, "profile")) { c->profile = value != 0; return UGKS_OK; }
     return fail(c, UGKS_EINVAL, "unknown option %s", name);
 }
 
@@ -249,16 +255,49 @@ int ugks_step(ugks_ctx *c, int n)
 {
     if (!c || n < 0) return fail(c, UGKS_EINVAL, "%s", "bad argument");
     if (!c->have_state) return fail(c, UGKS_ESTATE, "%s", "ugks_step before ugks_set_state");
+    if (c->profile) {
+        const int need = c->nev_used + 6 * n;
+        if (need > c->nev) {
+            cudaEvent_t *ne = (cudaEvent_t *)realloc(c->ev, sizeof(cudaEvent_t) * need);
+            if (!ne) return fail(c, UGKS_ENOMEM, "%s", "event pool");
+            c->ev = ne;
+            for (int i = c->nev; i < need; ++i) CK(cudaEventCreate(&c->ev[i]), "ugks_step(profile)");
+            c->nev = need;
+        }
+    }
     for (int s = 0; s < n; ++s) {
-        c->launches += launch_face_moments(c->P, c->cur, c->st);       // R, S1, S7 sums
+        cudaEvent_t *e = c->profile ? c->ev + c->nev_used : nullptr;
+        if (e) cudaEventRecord(e[0], c->st);
+        c->launches += launch_face_moments(c->P, c->cur, 0, c->st);    // R, S1, S7 sums, x-faces
+        if (e) cudaEventRecord(e[1], c->st);
+        c->launches += launch_face_moments(c->P, c->cur, 1, c->st);    // ... y-faces
+        if (e) cudaEventRecord(e[2], c->st);
         c->launches += launch_face_scalars(c->P, c->cur, c->st);       // S2..S5, wall density
+        if (e) cudaEventRecord(e[3], c->st);
         c->launches += launch_cell_scalars(c->P, c->cur, c->resblocks, c->st);   // U1, U2, residual partials
+        if (e) cudaEventRecord(e[4], c->st);
         c->launches += launch_flux_update(c->P, c->cur, c->st);        // S6, S8, U3
+        if (e) { cudaEventRecord(e[5], c->st); c->nev_used += 6; }
         c->cur ^= 1;
         c->steps += 1;
     }
     CK(cudaGetLastError(), "ugks_step");
     if (n > 0) c->have_res = 1;
+    return UGKS_OK;
+}
+
+int ugks_kernel_times(ugks_ctx *c, double ms[5], long counts[5])
+{
+    if (!c || !ms || !counts) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
+    CK(cudaStreamSynchronize(c->st), "ugks_kernel_times");
+    for (int i = 0; i + 5 < c->nev_used; i += 6)
+        for (int k = 0; k < 5; ++k) {
+            float t = 0.f;
+            CK(cudaEventElapsedTime(&t, c->ev[i + k], c->ev[i + k + 1]), "ugks_kernel_times");
+            c->kms[k] += t; c->kcnt[k] += 1;
+        }
+    c->nev_used = 0;
+    for (int k = 0; k < 5; ++k) { ms[k] = c->kms[k]; counts[k] = c->kcnt[k]; c->kms[k] = 0.0; c->kcnt[k] = 0; }
     return UGKS_OK;
 }
 

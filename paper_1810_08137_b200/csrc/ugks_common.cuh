@@ -110,7 +110,7 @@ __device__ __forceinline__ double warp_sum(double x)
 }
 
 // launchers (one per translation unit); each returns the number of kernels it enqueued
-int launch_face_moments(const UgksParams &P, int cur, cudaStream_t st);
+int launch_face_moments(const UgksParams &P, int cur, int dir, cudaStream_t st);
 int launch_face_scalars(const UgksParams &P, int cur, cudaStream_t st);
 int launch_cell_scalars(const UgksParams &P, int cur, int resblocks, cudaStream_t st);
 int launch_flux_update(const UgksParams &P, int cur, cudaStream_t st);

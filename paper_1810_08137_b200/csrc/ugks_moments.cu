@@ -175,19 +175,19 @@ size_t smem_face_moments(const UgksParams &P)
 
 static int block_threads(const UgksParams &P) { return ((P.Nu * P.R + 31) / 32) * 32; }
 
-int launch_face_moments(const UgksParams &P, int cur, cudaStream_t st)
+int launch_face_moments(const UgksParams &P, int cur, int dir, cudaStream_t st)
 {
     const size_t smem = smem_face_moments(P);
     const int nsx = (P.I + 1 + P.strip - 1) / P.strip, nsy = (P.J + 1 + P.strip - 1) / P.strip;
     const int T = block_threads(P);
     if (T <= 256) {
-        k_face_moments<0, 256><<<P.J * nsx * P.nchunk, T, smem, st>>>(P, cur);
-        k_face_moments<1, 256><<<P.I * nsy * P.nchunk, T, smem, st>>>(P, cur);
+        if (dir == 0) k_face_moments<0, 256><<<P.J * nsx * P.nchunk, T, smem, st>>>(P, cur);
+        else k_face_moments<1, 256><<<P.I * nsy * P.nchunk, T, smem, st>>>(P, cur);
     } else {
-        k_face_moments<0, 1024><<<P.J * nsx * P.nchunk, T, smem, st>>>(P, cur);
-        k_face_moments<1, 1024><<<P.I * nsy * P.nchunk, T, smem, st>>>(P, cur);
+        if (dir == 0) k_face_moments<0, 1024><<<P.J * nsx * P.nchunk, T, smem, st>>>(P, cur);
+        else k_face_moments<1, 1024><<<P.I * nsy * P.nchunk, T, smem, st>>>(P, cur);
     }
-    return 2;
+    return 1;
 }
 
 int setup_moments_attributes(const UgksParams &P)

@@ -136,7 +136,7 @@ def maxwellian_field(p: Problem, rho, U, V, T, out: np.ndarray | None = None) ->
     return f
 
 
-def initial_state(p: Problem, want_f: bool = True):
+def initial_state(p: Problem, want_f: bool = True, out_f: np.ndarray | None = None):
     """Seeded primitives -> (W[J][I][4], f[J][I][Nv][Nu], prim[J][I][4]) for problem ``p`` (AMB-18)."""
     rng = np.random.default_rng(p.seed)
     n = [smooth_noise(p, rng) for _ in range(4)]          # order rho, U, V, T
@@ -148,5 +148,5 @@ def initial_state(p: Problem, want_f: bool = True):
     lam = 1.0 / T
     W = np.stack([rho, rho * U, rho * V, 0.5 * rho * (U * U + V * V) + rho / (2.0 * lam)], axis=-1)
     prim = np.stack([rho, U, V, lam], axis=-1)
-    f = maxwellian_field(p, rho, U, V, T) if want_f else None
+    f = maxwellian_field(p, rho, U, V, T, out=out_f) if want_f else None
     return np.ascontiguousarray(W), f, prim

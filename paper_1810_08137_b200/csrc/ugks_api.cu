@@ -47,10 +47,18 @@ static void choose_geometry(int I, int J, int Nu, int Nv, int *chunk_m, int *R, 
     int cm = 800 / Nu; if (cm < 1) cm = 1;
     if (cm >= Nv) cm = Nv;
     else if ((Nu & 1) && (cm & 1)) cm += 1;                 // 16-byte aligned chunk starts for odd Nu
+    // R rows in parallel, NPT = ceil(cm/R) <= 8 points per thread: minimise issue slots (padded threads x NPT),
+    // prefer NPT near 4..5 (amortises the per-face per-thread setup without starving the SM of warps)
     int rmax = 256 / Nu; if (rmax < 1) rmax = 1; if (rmax > cm) rmax = cm;
-    int r = rmax;
-    for (int t = rmax; t >= 1 && 2 * t >= rmax; --t) if (cm % t == 0) { r = t; break; }
-    *chunk_m = cm; *R = r;
+    int best = rmax; long bestcost = -1;
+    for (int r = rmax; r >= 1; --r) {
+        const int npt = (cm + r - 1) / r;
+        if (npt > 8) break;
+        const long threads = ((long)Nu * r + 31) / 32 * 32;
+        const long cost = threads * npt * 16 + (npt < 4 ? (4 - npt) * 64 : (npt - 4) * 8);
+        if (bestcost < 0 || cost < bestcost) { bestcost = cost; best = r; }
+    }
+    *chunk_m = cm; *R = best;
     const int nchunk = (Nv + cm - 1) / cm;
     int s = 32;
     while (s > 8 && (long)J * ((I + s - 1) / s) * nchunk < 148L * 4) s >>= 1;
@@ -168,6 +176,7 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     c->st = (cudaStream_t)cuda_stream;
     choose_geometry(P.I, P.J, P.Nu, P.Nv, &P.chunk_m, &P.R, &P.strip);
     P.nchunk = (P.Nv + P.chunk_m - 1) / P.chunk_m;
+    P.npt = (P.chunk_m + P.R - 1) / P.R;
 
     double bcprim[16];
     for (int s = 0; s < 4; ++s) { bcprim[s * 4] = b[s]->rho; bcprim[s * 4 + 1] = b[s]->U; bcprim[s * 4 + 2] = b[s]->V; bcprim[s * 4 + 3] = b[s]->T; }
@@ -213,11 +222,12 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
     if (!strcmp(name, "chunk_m") || !strcmp(name, "R")) {
         int cm = P.chunk_m, R = P.R;
         if (!strcmp(name, "chunk_m")) cm = value; else R = value;
-        if (cm < 1 || cm > P.Nv || R < 1 || R > cm || P.Nu * R > 1024) return fail(c, UGKS_EINVAL, "%s", "chunk_m / R out of range");
+        if (cm < 1 || cm > P.Nv || R < 1 || P.Nu * R > 1024) return fail(c, UGKS_EINVAL, "%s", "chunk_m / R out of range");
         const int nchunk = (P.Nv + cm - 1) / cm;
         if (nchunk > c->nchunk_alloc) return fail(c, UGKS_EINVAL, "%s", "chunk_m too small for the allocated moment buffers");
         if (nchunk > 1 && ((cm * P.Nu) & 1)) return fail(c, UGKS_EINVAL, "%s", "chunk_m * Nu must be even (16-byte aligned chunks)");
-        UgksParams T = P; T.chunk_m = cm; T.R = R; T.nchunk = nchunk;
+        UgksParams T = P; T.chunk_m = cm; T.R = R; T.nchunk = nchunk; T.npt = (cm + R - 1) / R;
+        if (T.npt > 8) return fail(c, UGKS_EINVAL, "%s", "chunk_m / R must be <= 8 points per thread");
         if (smem_flux_update(T) > 227 * 1024) return fail(c, UGKS_EINVAL, "%s", "chunk does not fit in shared memory");
         P = T;
         if (setup_moments_attributes(P) || setup_update_attributes(P)) return cuda_fail(c, cudaGetLastError(), "ugks_set_option");

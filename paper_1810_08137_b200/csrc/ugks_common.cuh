@@ -10,13 +10,16 @@
 enum { BC_PERIODIC = 0, BC_FIXED = 1, BC_WALL = 2 };
 
 constexpr int NMOM = 12;    // per-(face,chunk) raw moments: 11 used, padded to 12
-constexpr int NCOEF = 28;   // per-face coefficients consumed by the flux/update kernel
+constexpr int NCOEF = 24;   // per-face coefficients consumed by the flux/update kernel
 constexpr int NCELL = 12;   // per-cell coefficients consumed by the flux/update kernel
-constexpr int RINGX = 6;    // stencil ring slots (4 live rows + 2 in flight)
+constexpr int RINGX = 6;    // face_moments: stencil ring slots (4 live rows + 2 in flight)
+constexpr int NSX = 4;      // flux_update: x-ring slots (2 live rows + 2 in flight; older rows live in registers)
 
 // coefficient record written by k_face_scalars (S2..S5) and read by k_flux_update (S6, S8)
-enum { CF_C0 = 0, CF_U = 1, CF_V = 2, CF_LAM = 3, CF_MT1 = 4, CF_MT2 = 5, CF_MT3 = 6, CF_MT4 = 7, CF_MT5 = 8,
-       CF_AL = 9, CF_AR = 13, CF_B = 17, CF_A = 21, CF_TYPE = 25, CF_RHOW = 26 };
+// P(n,t) = Mt1 + Mt2 (n a.psi + t b.psi) + Mt3 A.psi = sum c_ab n^a t^b (total degree <= 3); the five coefficients that
+// contain a (c10, c20, c30, c11, c12) come in an L (n > 0, a_L) and an R (n < 0, a_R) variant.
+enum { CF_C0 = 0, CF_U = 1, CF_V = 2, CF_LAM = 3, CF_MT4 = 4, CF_MT5 = 5, CF_RHOW = 6, CF_TYPE = 7,
+       CF_C00 = 8, CF_C01 = 9, CF_C02 = 10, CF_C03 = 11, CF_C21 = 12, CF_L = 13, CF_R = 18 };
 // per-cell record written by k_cell_scalars (U1, U2) and read by k_flux_update (U3)
 enum { CC_GN = 0, CC_UN = 1, CC_VN = 2, CC_LN = 3, CC_GP = 4, CC_UP = 5, CC_VP = 6, CC_LP = 7, CC_KF = 8, CC_KD = 9 };
 
@@ -41,6 +44,7 @@ struct UgksParams {
     int chunk_m;                     // velocity rows (m) per chunk
     int nchunk;                      // chunks per row of f
     int R;                           // m-rows processed in parallel by one CTA (blockDim = Nu*R)
+    int npt;                         // velocity points per thread = ceil(chunk_m / R), 1..8 (template parameter)
 };
 
 static __host__ __device__ inline int nfaces_x(const UgksParams &P) { return (P.I + 1) * P.J; }

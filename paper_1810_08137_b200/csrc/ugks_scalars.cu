@@ -187,9 +187,22 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
     for (int r = 0; r < 4; ++r) fw[r] = F[r];
 
     cf[CF_C0] = p0.rho * p0.lam / UGKS_PI; cf[CF_U] = p0.U; cf[CF_V] = p0.V; cf[CF_LAM] = p0.lam;
-    cf[CF_MT1] = Mt1; cf[CF_MT2] = Mt2; cf[CF_MT3] = Mt3; cf[CF_MT4] = Mt4; cf[CF_MT5] = Mt5;
-    for (int r = 0; r < 4; ++r) { cf[CF_AL + r] = aL[r]; cf[CF_AR + r] = aR[r]; cf[CF_B + r] = bb[r]; cf[CF_A + r] = A[r]; }
-    cf[CF_TYPE] = 0.0; cf[CF_RHOW] = 0.0; cf[27] = tau;
+    cf[CF_MT4] = Mt4; cf[CF_MT5] = Mt5; cf[CF_RHOW] = 0.0; cf[CF_TYPE] = 0.0;
+    cf[CF_C00] = Mt1 + Mt3 * A[0];
+    cf[CF_C01] = Mt2 * bb[0] + Mt3 * A[2];
+    cf[CF_C02] = Mt2 * bb[2] + 0.5 * Mt3 * A[3];
+    cf[CF_C03] = 0.5 * Mt2 * bb[3];
+    cf[CF_C21] = 0.5 * Mt2 * bb[3];
+    for (int sd = 0; sd < 2; ++sd) {
+        const double *a = sd == 0 ? aL : aR;
+        double *o = cf + (sd == 0 ? CF_L : CF_R);
+        o[0] = Mt2 * a[0] + Mt3 * A[1];              // c10
+        o[1] = Mt2 * a[1] + 0.5 * Mt3 * A[3];        // c20
+        o[2] = 0.5 * Mt2 * a[3];                     // c30
+        o[3] = Mt2 * (a[2] + bb[1]);                 // c11
+        o[4] = 0.5 * Mt2 * a[3];                     // c12
+    }
+    cf[23] = tau;
 }
 
 __global__ void __launch_bounds__(128) k_face_scalars(const UgksParams P, const int cur)

@@ -12,9 +12,10 @@
 //   * the x-face flux is evaluated once per face and carried in registers to the next cell; the two y-faces of
 //     a cell are evaluated by the cell.  f^{n+1} is written straight from registers: f crosses HBM once each way.
 #include "ugks_common.cuh"
+#include <type_traits>
 
 constexpr int REC_X = 0, REC_YL = NCOEF, REC_YU = 2 * NCOEF, REC_CC = 3 * NCOEF, REC_SIZE = 3 * NCOEF + NCELL;   // 84
-constexpr int NREC = 3;                                              // record slots: records arrive two steps ahead
+constexpr int NREC = 4;                                              // record slots: records arrive three steps ahead
 // per-step table buffer (doubles): k-tables [6 x-face][7 y-lower][7 y-upper][2 relaxation] x Nu, then
 // m-tables [x-face Et][y-lower En][y-upper En][g^n][g^{n+1}] x chunk_m
 constexpr int TK_X = 0, TK_YL = 6, TK_YU = 13, TK_G = 20, NKT = 22, NMT = 5;
@@ -81,7 +82,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_flux_update(const UgksParams P, 
     double *ybuf = ring + (size_t)NSX * Qs;                          // [2][4][Qs]
     double *tabs = ybuf + (size_t)8 * Qs;                            // [2][tabsz]
     double *recs = tabs + 2 * tabsz;                                 // [NREC][REC_SIZE]
-    uint64_t *bars = reinterpret_cast<uint64_t *>(recs + NREC * REC_SIZE);   // [NSX] x-ring, [2] y buffers, [NREC] records
+    double *un = recs + NREC * REC_SIZE;                             // [Nu] velocity nodes u_k
+    double *vn = un + ((Nu + 1) & ~1);                               // [CM] velocity nodes v_m of this chunk
+    uint64_t *bars = reinterpret_cast<uint64_t *>(vn + ((CM + 1) & ~1));     // [NSX] x-ring, [2] y buffers, [NREC] records
 
     const int tid = threadIdx.x;
     const bool active = tid < Nu * R;
@@ -127,63 +130,65 @@ __global__ void __launch_bounds__(MAXT, MINB) k_flux_update(const UgksParams P, 
             tma_load_1d(dst + REC_CC, P.cellc + ((size_t)j * P.I + cell) * NCELL, NCELL * 8, &bars[NSX + 2 + sl]);
         }
     };
-    // tables of step st -> buffer st&1.  One work item = one velocity node of one table group:
-    //   items [0,3Nu): (face f, k): separable factor E[k] and the flux polynomial column of that face at u_k
-    //   items [3Nu,5Nu): relaxation factors of g^n, g^{n+1} in u;  items [5Nu, 5Nu+5mc): the five m-tables
+    // tables of step st -> buffer st&1, two warp-uniform groups of work items:
+    //   A (threads from the front): one item per (face f, k): E[k] and the flux-polynomial column of that face at u_k
+    //   B (threads from the back): one item per plain separable factor: g^n, g^{n+1} in u (2 Nu) and the five m-tables
     auto make_tables = [&](int st) {
         const int sl = (st - c0) % NREC;
         mbar_wait(&bars[NSX + 2 + sl], ((st - c0) / NREC) & 1);
         const double *rec = recs + sl * REC_SIZE;
         double *T = tabs + (size_t)(st & 1) * tabsz, *Tm = T + NKT * Nu;
         const bool have_cell = st > c0;
-        const int nitem = 5 * Nu + 5 * mc;
-        for (int e = tid; e < nitem; e += blockDim.x) {
-            if (e < 3 * Nu) {
-                const int f = e / Nu, kk = e - f * Nu;
-                if (f > 0 && !have_cell) continue;
-                const double *g = rec + f * NCOEF;
-                const double c = P.u[kk];
-                if (f == 0) {                                        // x-face: n = u_k, cubic in t
-                    const double *LR = g + (c > 0.0 ? CF_L : CF_R);
-                    const double d = c - g[CF_U];
-                    const double sc = P.dy * c * g[CF_C0] * exp(-g[CF_LAM] * d * d);
-                    double *o = T + TK_X * Nu + kk;
-                    o[0] = sc * fma(c, fma(c, fma(c, LR[2], LR[1]), LR[0]), g[CF_C00]);
-                    o[Nu] = sc * fma(c, fma(c, g[CF_C21], LR[3]), g[CF_C01]);
-                    o[2 * Nu] = sc * fma(c, LR[4], g[CF_C02]);
-                    o[3 * Nu] = sc * g[CF_C03];
-                    o[4 * Nu] = P.dy * c * g[CF_MT4];
-                    o[5 * Nu] = -P.dy * c * c * g[CF_MT5] * ihx;
-                } else {                                             // y-face: t = u_k, cubic in n (L and R variants)
-                    const double d = c - g[CF_V];
-                    const double sc = P.dx * exp(-g[CF_LAM] * d * d);
-                    const double *L = g + CF_L, *Rr = g + CF_R;
-                    double *o = T + (f == 1 ? TK_YL : TK_YU) * Nu + kk;
-                    o[0] = sc * fma(c, fma(c, fma(c, g[CF_C03], g[CF_C02]), g[CF_C01]), g[CF_C00]);
-                    o[Nu] = sc * fma(c, fma(c, L[4], L[3]), L[0]);
-                    o[2 * Nu] = sc * fma(c, g[CF_C21], L[1]);
-                    o[3 * Nu] = sc * L[2];
-                    o[4 * Nu] = sc * fma(c, fma(c, Rr[4], Rr[3]), Rr[0]);
-                    o[5 * Nu] = sc * fma(c, g[CF_C21], Rr[1]);
-                    o[6 * Nu] = sc * Rr[2];
-                }
-            } else if (e < 5 * Nu) {
-                if (!have_cell) continue;
-                const int w = (e - 3 * Nu) / Nu, kk = e - (3 + w) * Nu;
-                const double *cc = rec + REC_CC + (w == 0 ? CC_GN : CC_GP);
-                const double d = P.u[kk] - cc[1];
-                T[(TK_G + w) * Nu + kk] = cc[0] * exp(-cc[3] * d * d);
-            } else {
-                const int e2 = e - 5 * Nu, tab = e2 / mc, mi = e2 - tab * mc;
-                if (tab > 0 && !have_cell) continue;
-                const double vv = P.v[m0 + mi];
-                double pref, lam, cen;
-                if (tab == 0) { pref = 1.0; lam = rec[REC_X + CF_LAM]; cen = rec[REC_X + CF_V]; }
-                else if (tab <= 2) { const double *g = rec + tab * NCOEF; pref = g[CF_C0]; lam = g[CF_LAM]; cen = g[CF_U]; }
-                else { const double *cc = rec + REC_CC + (tab == 3 ? CC_GN : CC_GP); pref = 1.0; lam = cc[3]; cen = cc[2]; }
-                const double d = vv - cen;
-                Tm[tab * CM + mi] = pref * exp(-lam * d * d);
+        const int nA = (have_cell ? 3 : 1) * Nu;
+        for (int e = tid; e < nA; e += blockDim.x) {
+            const int f = (e >= Nu) + (e >= 2 * Nu), kk = e - f * Nu;
+            const double *g = rec + f * NCOEF;
+            const double c = un[kk];
+            const double d = c - (f == 0 ? g[CF_U] : g[CF_V]);
+            const double E = exp(-g[CF_LAM] * d * d);
+            if (f == 0) {                                            // x-face: n = u_k, cubic in t
+                const double *LR = g + (c > 0.0 ? CF_L : CF_R);
+                const double sc = P.dy * c * g[CF_C0] * E;
+                double *o = T + TK_X * Nu + kk;
+                o[0] = sc * fma(c, fma(c, fma(c, LR[2], LR[1]), LR[0]), g[CF_C00]);
+                o[Nu] = sc * fma(c, fma(c, g[CF_C21], LR[3]), g[CF_C01]);
+                o[2 * Nu] = sc * fma(c, LR[4], g[CF_C02]);
+                o[3 * Nu] = sc * g[CF_C03];
+                o[4 * Nu] = P.dy * c * g[CF_MT4];
+                o[5 * Nu] = -P.dy * c * c * g[CF_MT5] * ihx;
+            } else {                                                 // y-face: t = u_k, cubic in n (L and R variants)
+                const double sc = P.dx * E;
+                const double *L = g + CF_L, *Rr = g + CF_R;
+                double *o = T + (f == 1 ? TK_YL : TK_YU) * Nu + kk;
+                o[0] = sc * fma(c, fma(c, fma(c, g[CF_C03], g[CF_C02]), g[CF_C01]), g[CF_C00]);
+                o[Nu] = sc * fma(c, fma(c, L[4], L[3]), L[0]);
+                o[2 * Nu] = sc * fma(c, g[CF_C21], L[1]);
+                o[3 * Nu] = sc * L[2];
+                o[4 * Nu] = sc * fma(c, fma(c, Rr[4], Rr[3]), Rr[0]);
+                o[5 * Nu] = sc * fma(c, g[CF_C21], Rr[1]);
+                o[6 * Nu] = sc * Rr[2];
             }
+        }
+        // B items: [0, mc): x-face Et[m];  then (cell only) y-lower En[m], y-upper En[m], g^n v, g^{n+1} v, g^n u, g^{n+1} u
+        const int nB = have_cell ? 5 * mc + 2 * Nu : mc;
+        for (int e = (int)blockDim.x - 1 - tid; e < nB; e += blockDim.x) {
+            const bool isk = e >= 5 * mc;
+            const int e2 = isk ? e - 5 * mc : e;
+            const int len = isk ? Nu : mc;
+            int tab = 0;
+            tab += e2 >= len; tab += e2 >= 2 * len; tab += e2 >= 3 * len; tab += e2 >= 4 * len;
+            const int idx = e2 - tab * len;
+            const double node = isk ? un[idx] : vn[idx];
+            // (pref, lam, centre) of the factor
+            const bool relax = isk || tab >= 3;
+            const int w = isk ? tab : tab - 3;                       // 0: g^n, 1: g^{n+1}
+            const double *g = relax ? rec + REC_CC + (w == 0 ? CC_GN : CC_GP) : rec + tab * NCOEF;
+            const double lam = relax ? g[3] : g[CF_LAM];
+            const double cen = relax ? (isk ? g[1] : g[2]) : (tab == 0 ? g[CF_V] : g[CF_U]);
+            const double pref = relax ? (isk ? g[0] : 1.0) : (tab == 0 ? 1.0 : g[CF_C0]);
+            const double d = node - cen;
+            const double val = pref * exp(-lam * d * d);
+            if (isk) T[(TK_G + tab) * Nu + idx] = val; else Tm[tab * CM + idx] = val;
         }
     };
 
@@ -191,10 +196,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_flux_update(const UgksParams P, 
         for (int i = 0; i < NSX + 2 + NREC; ++i) mbar_init(&bars[i], 1);
         mbar_fence_init();
     }
+    for (int i = tid; i < Nu; i += blockDim.x) un[i] = P.u[i];
+    for (int i = tid; i < mc; i += blockDim.x) vn[i] = P.v[m0 + i];
     __syncthreads();
     if (tid == 0) {
         issue_rec(c0);
         issue_rec(c0 + 1);
+        if (c0 + 2 <= c1) issue_rec(c0 + 2);
         for (int row = rows_first; row < rows_first + NSX && row <= rows_last; ++row) issue_x(row);
         issue_y(c0);
         if (c0 + 1 < c1) issue_y(c0 + 1);
@@ -204,24 +212,25 @@ __global__ void __launch_bounds__(MAXT, MINB) k_flux_update(const UgksParams P, 
     const double uk = active ? P.u[k] : 0.0;
     const bool posx = uk > 0.0;
     const double sgx = posx ? 1.0 : -1.0;
+    // Per-thread points p = 0..NPT-1: velocity row m = r + p R.  A point outside the chunk (ragged tail, padding
+    // threads) is clamped onto point 0 of the row so that the arithmetic stays branch-free; only its store is masked.
     double vreg[NPT], fm[NPT], fc[NPT], Fprev[NPT];
     bool valid[NPT];
+    int qo[NPT], mo[NPT];
 #pragma unroll
     for (int p = 0; p < NPT; ++p) {
         const int mm = r + p * R;
         valid[p] = active && mm < mc;
-        vreg[p] = valid[p] ? P.v[m0 + mm] : 0.0;
+        qo[p] = valid[p] ? mm * Nu + k : 0;
+        mo[p] = valid[p] ? mm : 0;
+        vreg[p] = vn[mo[p]];
         Fprev[p] = 0.0;
     }
-    const int qbase = r * Nu + k, qstep = R * Nu;
     {   // prologue: the two oldest rows of each thread's x-window go to registers
         wait_x(c0 - 2); wait_x(c0 - 1); wait_x(c0);
         const double *ra = ring + (size_t)(posx ? 0 : 1) * Qs, *rb = ring + (size_t)(posx ? 1 : 2) * Qs;
 #pragma unroll
-        for (int p = 0; p < NPT; ++p) {
-            fm[p] = valid[p] ? ra[qbase + p * qstep] : 0.0;
-            fc[p] = valid[p] ? rb[qbase + p * qstep] : 0.0;
-        }
+        for (int p = 0; p < NPT; ++p) { fm[p] = ra[qo[p]]; fc[p] = rb[qo[p]]; }
     }
     __syncthreads();                                                 // tables of step c0 complete; rows c0-2, c0-1 consumed
     if (tid == 0) {
@@ -241,96 +250,79 @@ __global__ void __launch_bounds__(MAXT, MINB) k_flux_update(const UgksParams P, 
         {
             const int ms = miss_mask<0>(P, a);
             const int sh = posx ? 0 : 1;
-            const bool mm_ = (ms >> sh) & 1, mc_ = (ms >> (sh + 1)) & 1, mp_ = (ms >> (sh + 2)) & 1;
             const double *rn = ring + (size_t)((a + sh - rows_first) % NSX) * Qs;
             const double *tk = T + TK_X * Nu + k;
             const double p0 = tk[0], p1 = tk[Nu], p2 = tk[2 * Nu], p3 = tk[3 * Nu], c4 = tk[4 * Nu], c5 = tk[5 * Nu];
-            const double rw = rec[REC_X + CF_RHOW];
-            const double *gw = P.wallg + (size_t)(posx ? 0 : 1) * P.Npad + q0;
+            auto xpass = [&](auto fl) {
+                constexpr bool FL = decltype(fl)::value;
+                const bool mm_ = (ms >> sh) & 1, mc_ = (ms >> (sh + 1)) & 1, mp_ = (ms >> (sh + 2)) & 1;
+                const double rw = rec[REC_X + CF_RHOW];
+                const double *gw = P.wallg + (size_t)(posx ? 0 : 1) * P.Npad + q0;
 #pragma unroll
-            for (int p = 0; p < NPT; ++p) {
-                if (valid[p]) {
-                    const int q = qbase + p * qstep;
-                    const double fn = rn[q], t = vreg[p];
+                for (int p = 0; p < NPT; ++p) {
+                    const double fn = rn[qo[p]], t = vreg[p];
                     double f0, hs;
-                    if (ms == 0) recon<false>(fm[p], fc[p], fn, sgx, false, false, false, 0.0, f0, hs);
-                    else recon<true>(fm[p], fc[p], fn, sgx, mm_, mc_, mp_, mc_ ? rw * gw[q] : 0.0, f0, hs);
-                    const double X = fma(t, fma(t, fma(t, p3, p2), p1), p0) * Tm[p * R + r];
+                    recon<FL>(fm[p], fc[p], fn, sgx, mm_, mc_, mp_, (FL && mc_) ? rw * gw[qo[p]] : 0.0, f0, hs);
+                    const double X = fma(t, fma(t, fma(t, p3, p2), p1), p0) * Tm[mo[p]];
                     const double F = fma(c4, f0, fma(c5, hs, X));
                     D[p] = Fprev[p] - F;
                     Fprev[p] = F;
                     own[p] = posx ? fc[p] : fm[p];                   // row of cell a-1
                     fm[p] = fc[p]; fc[p] = fn;
                 }
-            }
+            };
+            if (ms == 0) xpass(std::false_type{}); else xpass(std::true_type{});
         }
         if (a > c0) {
             const int cell = a - 1, buf = (cell - c0) & 1;
             mbar_wait(&bars[NSX + buf], ((cell - c0) >> 1) & 1);
             const double *y0 = ybuf + (size_t)(buf * 4) * Qs, *y1 = y0 + Qs, *y3 = y1 + Qs, *y4 = y3 + Qs;
-            {   // lower face j
-                const double *tk = T + TK_YL * Nu + k;
-                const double q0_ = tk[0], q1L = tk[Nu], q2L = tk[2 * Nu], q3L = tk[3 * Nu], q1R = tk[4 * Nu], q2R = tk[5 * Nu], q3R = tk[6 * Nu];
-                const double c4 = P.dx * rec[REC_YL + CF_MT4], c5 = -P.dx * rec[REC_YL + CF_MT5] * ihy, rw = rec[REC_YL + CF_RHOW];
-#pragma unroll
-                for (int p = 0; p < NPT; ++p) {
-                    if (valid[p]) {
-                        const int q = qbase + p * qstep;
-                        const double n = vreg[p], o = own[p], a1 = y1[q];
-                        const bool pos = n > 0.0;
-                        double f0, hs;
-                        if (pos) {
-                            const double a0 = y0[q];
-                            if (!anyms) recon<false>(a0, a1, o, 1.0, false, false, false, 0.0, f0, hs);
-                            else recon<true>(a0, a1, o, 1.0, msy0 & 1, msy0 & 2, msy0 & 4, (msy0 & 2) ? rw * gwy0[q] : 0.0, f0, hs);
-                        } else {
-                            const double a3 = y3[q];
-                            if (!anyms) recon<false>(a1, o, a3, -1.0, false, false, false, 0.0, f0, hs);
-                            else recon<true>(a1, o, a3, -1.0, msy0 & 2, msy0 & 4, msy0 & 8, 0.0, f0, hs);
-                        }
-                        const double q1 = pos ? q1L : q1R, q2 = pos ? q2L : q2R, q3 = pos ? q3L : q3R;
-                        const double poly = fma(n, fma(n, fma(n, q3, q2), q1), q0_);
-                        D[p] += n * fma(c4, f0, fma(c5 * n, hs, poly * Tm[CM + p * R + r]));
-                    }
+            // one y-face: UP = 0 lower face j (rows j-2..j+1), UP = 1 upper face j+1 (rows j-1..j+2); returns its flux
+            auto yflux = [&](auto fl, auto up, int p, const double *tk, double c4, double c5, double rw, int ms, const double *gwy) {
+                constexpr bool FL = decltype(fl)::value;
+                constexpr int UP = decltype(up)::value;
+                const double n = vreg[p], o = own[p];
+                const int q = qo[p];
+                const bool pos = n > 0.0;
+                double f0, hs;
+                if (pos) {                                           // upwind cell is the lower one of the face
+                    const double lo = UP ? y1[q] : y0[q], mid = UP ? o : y1[q], hi = UP ? y3[q] : o;
+                    recon<FL>(lo, mid, hi, 1.0, ms & 1, ms & 2, ms & 4, (FL && (ms & 2)) ? rw * gwy[q] : 0.0, f0, hs);
+                } else {
+                    const double lo = UP ? o : y1[q], mid = UP ? y3[q] : o, hi = UP ? y4[q] : y3[q];
+                    recon<FL>(lo, mid, hi, -1.0, ms & 2, ms & 4, ms & 8, (FL && (ms & 4)) ? rw * gwy[q] : 0.0, f0, hs);
                 }
-            }
-            {   // upper face j+1, then the update of the cell
+                const double q1 = pos ? tk[Nu] : tk[4 * Nu], q2 = pos ? tk[2 * Nu] : tk[5 * Nu], q3 = pos ? tk[3 * Nu] : tk[6 * Nu];
+                const double poly = fma(n, fma(n, fma(n, q3, q2), q1), tk[0]);
+                return n * fma(c4, f0, fma(c5 * n, hs, poly * Tm[(1 + UP) * CM + mo[p]]));
+            };
+            auto ypass = [&](auto fl) {
+                {
+                    const double *tk = T + TK_YL * Nu + k;
+                    const double c4 = P.dx * rec[REC_YL + CF_MT4], c5 = -P.dx * rec[REC_YL + CF_MT5] * ihy, rw = rec[REC_YL + CF_RHOW];
+#pragma unroll
+                    for (int p = 0; p < NPT; ++p) D[p] += yflux(fl, std::integral_constant<int, 0>{}, p, tk, c4, c5, rw, msy0, gwy0);
+                }
                 const double *tk = T + TK_YU * Nu + k;
-                const double q0_ = tk[0], q1L = tk[Nu], q2L = tk[2 * Nu], q3L = tk[3 * Nu], q1R = tk[4 * Nu], q2R = tk[5 * Nu], q3R = tk[6 * Nu];
                 const double c4 = P.dx * rec[REC_YU + CF_MT4], c5 = -P.dx * rec[REC_YU + CF_MT5] * ihy, rw = rec[REC_YU + CF_RHOW];
                 const double gnu = T[TK_G * Nu + k], gpu = T[(TK_G + 1) * Nu + k];
                 const double KF = rec[REC_CC + CC_KF], KD = rec[REC_CC + CC_KD];
                 double *out = fnew + ((size_t)j * P.I + cell) * P.Npad + q0;
 #pragma unroll
                 for (int p = 0; p < NPT; ++p) {
-                    if (valid[p]) {
-                        const int q = qbase + p * qstep, mi = p * R + r;
-                        const double n = vreg[p], o = own[p], a3 = y3[q];
-                        const bool pos = n > 0.0;
-                        double f0, hs;
-                        if (pos) {
-                            const double a1 = y1[q];
-                            if (!anyms) recon<false>(a1, o, a3, 1.0, false, false, false, 0.0, f0, hs);
-                            else recon<true>(a1, o, a3, 1.0, msy1 & 1, msy1 & 2, msy1 & 4, 0.0, f0, hs);
-                        } else {
-                            const double a4 = y4[q];
-                            if (!anyms) recon<false>(o, a3, a4, -1.0, false, false, false, 0.0, f0, hs);
-                            else recon<true>(o, a3, a4, -1.0, msy1 & 2, msy1 & 4, msy1 & 8, (msy1 & 4) ? rw * gwy1[q] : 0.0, f0, hs);
-                        }
-                        const double q1 = pos ? q1L : q1R, q2 = pos ? q2L : q2R, q3 = pos ? q3L : q3R;
-                        const double poly = fma(n, fma(n, fma(n, q3, q2), q1), q0_);
-                        const double Dq = D[p] - n * fma(c4, f0, fma(c5 * n, hs, poly * Tm[2 * CM + mi]));
-                        const double g = fma(Tm[4 * CM + mi], gpu, Tm[3 * CM + mi] * gnu);
-                        out[q] = fma(KF, o, fma(KD, Dq, g));         // P:L41 Eq. (3), solved for f^{n+1}
-                    }
+                    const double Dq = D[p] - yflux(fl, std::integral_constant<int, 1>{}, p, tk, c4, c5, rw, msy1, gwy1);
+                    const double g = fma(Tm[4 * CM + mo[p]], gpu, Tm[3 * CM + mo[p]] * gnu);
+                    const double fnw = fma(KF, own[p], fma(KD, Dq, g));       // P:L41 Eq. (3), solved for f^{n+1}
+                    if (valid[p]) out[qo[p]] = fnw;
                 }
-            }
+            };
+            if (!anyms) ypass(std::false_type{}); else ypass(std::true_type{});
         }
         __syncthreads();
         if (tid == 0) {
             if (a + NSX <= rows_last) issue_x(a + NSX);              // row a is consumed, its slot takes row a+4
             if (a > c0 && a + 1 < c1) issue_y(a + 1);
-            if (a + 2 <= c1) issue_rec(a + 2);
+            if (a + 3 <= c1) issue_rec(a + 3);
         }
     }
 }
@@ -339,7 +331,8 @@ size_t smem_flux_update(const UgksParams &P)
 {
     const size_t Qs = ((size_t)P.chunk_m * P.Nu + 1) & ~(size_t)1;
     const size_t tabsz = ((size_t)NKT * P.Nu + (size_t)NMT * P.chunk_m + 1) & ~(size_t)1;
-    return ((NSX + 8) * Qs + 2 * tabsz + NREC * REC_SIZE) * sizeof(double) + (NSX + 2 + NREC) * sizeof(uint64_t);
+    return ((NSX + 8) * Qs + 2 * tabsz + NREC * REC_SIZE + (((size_t)P.Nu + 1) & ~(size_t)1) + (((size_t)P.chunk_m + 1) & ~(size_t)1)) * sizeof(double)
+           + (NSX + 2 + NREC) * sizeof(uint64_t);
 }
 
 // thread-count classes: <=128 threads (4 CTAs/SM by registers), <=256 (2 CTAs/SM), <=1024 (1 CTA/SM)

@@ -14,6 +14,7 @@
 #include <type_traits>
 
 constexpr int NACC = 7;
+constexpr int NSM = 4;       // stencil ring slots: 2 live rows + 2 in flight (8 slots measured no faster: not latency-bound)
 
 __device__ __forceinline__ double vl_half_rcp(double dm, double dp)
 {
@@ -72,14 +73,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_face_moments(const UgksParams P,
     const uint32_t bytes = (uint32_t)(((Q + 1) & ~1) * sizeof(double));
     const int B = blockDim.x;
 
-    double *ring = reinterpret_cast<double *>(smem_raw);            // [NSX][Qs]
-    double *part = ring + (size_t)NSX * Qs;                         // [2][NACC][B]   per-thread partial sums
+    double *ring = reinterpret_cast<double *>(smem_raw);            // [NSM][Qs]
+    double *part = ring + (size_t)NSM * Qs;                         // [2][NACC][B]   per-thread partial sums
     double *col = part + 2 * NACC * B;                              // [2][NACC][Nu]  per-column sums
     double *un = col + 2 * NACC * Nu;                               // [Nu] u_k, then [Nu] wu_k
     double *wun = un + Nu;
     double *vn = wun + Nu;                                          // [CM] v_m, then [CM] wv_m
     double *wvn = vn + CM;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(wvn + CM);
+    double *red = wvn + CM;                                         // [2][32][16] per-warp moment sums
+    uint64_t *bars = reinterpret_cast<uint64_t *>(red + 2 * 32 * 16);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = B >> 5;
     const bool active = tid < Nu * R;
@@ -89,25 +91,25 @@ __global__ void __launch_bounds__(MAXT, MINB) k_face_moments(const UgksParams P,
 
     auto issue = [&](int row) {
         int miss;
-        const int sl = (row - rows_first) % NSX;
+        const int sl = (row - rows_first) % NSM;
         const double *src = row_ptr<DIR>(P, fcur, row, line, &miss) + q0;
         mbar_expect_tx(&bars[sl], bytes);
         tma_load_1d(ring + (size_t)sl * Qs, src, bytes, &bars[sl]);
     };
     auto wait_row = [&](int row) {
         const int idx = row - rows_first;
-        mbar_wait(&bars[idx % NSX], (idx / NSX) & 1);
+        mbar_wait(&bars[idx % NSM], (idx / NSM) & 1);
     };
 
     if (tid == 0) {
-        for (int i = 0; i < NSX; ++i) mbar_init(&bars[i], 1);
+        for (int i = 0; i < NSM; ++i) mbar_init(&bars[i], 1);
         mbar_fence_init();
     }
     for (int i = tid; i < Nu; i += B) { un[i] = P.u[i]; wun[i] = P.wu[i]; }
     for (int i = tid; i < mc; i += B) { vn[i] = P.v[m0 + i]; wvn[i] = P.wv[m0 + i]; }
     __syncthreads();
     if (tid == 0)
-        for (int row = rows_first; row < rows_first + NSX && row <= rows_last; ++row) issue(row);
+        for (int row = rows_first; row < rows_first + NSM && row <= rows_last; ++row) issue(row);
 
     const double uk = un[k];
     // per-thread points; points outside the chunk are clamped onto a valid one and get zero weight
@@ -134,16 +136,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_face_moments(const UgksParams P,
     }
     __syncthreads();
     if (tid == 0) {
-        if (a0 + 2 <= rows_last) issue(a0 + 2);
-        if (a0 + 3 <= rows_last) issue(a0 + 3);
+        if (a0 + NSM - 2 <= rows_last) issue(a0 + NSM - 2);
+        if (a0 + NSM - 1 <= rows_last) issue(a0 + NSM - 1);
     }
     const double inv_h = 2.0 / (DIR == 0 ? P.dx : P.dy);
 
-    for (int a = a0; a < a1 + 2; ++a) {
+    const int nw3 = min(nwarp, (Nu + 31) / 32);                     // warps that own columns in stage 3
+    for (int a = a0; a < a1 + 3; ++a) {
         if (a < a1) {                                               // stage 1: point sums of face a
             wait_row(a + 1);
-            const double *rA = ring + (size_t)((a - rows_first) % NSX) * Qs;          // row a
-            const double *rB = ring + (size_t)((a + 1 - rows_first) % NSX) * Qs;      // row a+1
+            const double *rA = ring + (size_t)((a - rows_first) % NSM) * Qs;          // row a
+            const double *rB = ring + (size_t)((a + 1 - rows_first) % NSM) * Qs;      // row a+1
             const int ms = miss_mask_m<DIR>(P, a);
             double acc[NACC];
 #pragma unroll
@@ -191,12 +194,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_face_moments(const UgksParams P,
                 cc[idx] = sum;
             }
         }
-        if (a - 2 >= a0 && warp == nwarp - 1) {                     // stage 3 (one warp): k-dependent factors + butterfly
+        if (a - 2 >= a0 && a - 2 < a1 && warp < nw3) {              // stage 3: k-dependent factors + butterfly, per warp
             const double *cc = col + (size_t)(a & 1) * NACC * Nu;   // (a-2)&1 == a&1
             double o[16];
 #pragma unroll
             for (int v = 0; v < 16; ++v) o[v] = 0.0;
-            for (int kk = lane; kk < Nu; kk += 32) {
+            for (int kk = tid; kk < Nu; kk += 32 * nw3) {
                 const double w = wun[kk], c = un[kk], c2 = c * c, ws = w * inv_h;
                 const double A0 = cc[kk], A1 = cc[Nu + kk], A2 = cc[2 * Nu + kk], A3 = cc[3 * Nu + kk];
                 const double B4 = cc[4 * Nu + kk], B5 = cc[5 * Nu + kk], B6 = cc[6 * Nu + kk];
@@ -240,14 +243,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_face_moments(const UgksParams P,
             o[0] += __shfl_xor_sync(0xffffffffu, o[0], 1);
             // lane holds moment v = 8*bit4 + 4*bit3 + 2*bit2 + bit1
             const int v = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
-            if ((lane & 1) == 0 && v < 11) {
-                const int fa = a - 2;
-                const size_t face = DIR == 0 ? (size_t)line * (P.I + 1) + fa : (size_t)fa * P.I + line;
-                P.mom[DIR][(face * P.nchunk + chunk) * NMOM + v] = o[0];
-            }
+            if ((lane & 1) == 0) red[((a & 1) * 32 + warp) * 16 + v] = o[0];
+        }
+        if (a - 3 >= a0 && tid < 11) {                              // stage 4: sum over the warps of stage 3, store
+            const double *rr = red + (size_t)((a - 1) & 1) * 32 * 16 + tid;   // (a-3)&1 == (a-1)&1
+            double sum = 0.0;
+            for (int w = 0; w < nw3; ++w) sum += rr[w * 16];
+            const int fa = a - 3;
+            const size_t face = DIR == 0 ? (size_t)line * (P.I + 1) + fa : (size_t)fa * P.I + line;
+            P.mom[DIR][(face * P.nchunk + chunk) * NMOM + tid] = sum;
         }
         __syncthreads();
-        if (tid == 0 && a < a1 && a + NSX <= rows_last) issue(a + NSX);   // row a is consumed by every thread
+        if (tid == 0 && a < a1 && a + NSM <= rows_last) issue(a + NSM);   // row a is consumed by every thread
     }
 }
 
@@ -256,7 +263,7 @@ size_t smem_face_moments(const UgksParams &P)
     const size_t Qs = ((size_t)P.chunk_m * P.Nu + 1) & ~(size_t)1;
     const size_t B = ((size_t)P.Nu * P.R + 31) / 32 * 32;
     const size_t tabs = 2 * (size_t)P.Nu + 2 * (size_t)P.chunk_m;
-    return (NSX * Qs + 2 * NACC * B + 2 * NACC * (size_t)P.Nu + tabs) * sizeof(double) + NSX * sizeof(uint64_t);
+    return (NSM * Qs + 2 * NACC * B + 2 * NACC * (size_t)P.Nu + tabs + 2 * 32 * 16) * sizeof(double) + NSM * sizeof(uint64_t);
 }
 
 static int block_threads(const UgksParams &P) { return ((P.Nu * P.R + 31) / 32) * 32; }

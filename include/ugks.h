@@ -38,7 +38,7 @@ enum { UGKS_BC_PERIODIC = 0, UGKS_BC_FIXED = 1, UGKS_BC_WALL = 2 };
 /* Uniform Cartesian mesh of I x J control volumes.  I, J >= 2. */
 typedef struct { int I, J; double x0, x1, y0, y1; } ugks_mesh;
 /* Discrete velocity grid K x M of the paper = Nu x Nv here.  HOST arrays, copied at init.
- * 1 <= Nu <= 1024, Nv >= 1.  Weights must have positive sums. */
+ * 1 <= Nu <= 256, Nv >= 1.  Weights must have positive sums. */
 typedef struct { int Nu, Nv; const double *u, *wu, *v, *wv; } ugks_vgrid;
 /* Gas: viscosity exponent omega (mu = mu_ref T^omega), mu_ref (<= 0: derive from Kn, AMB-7),
  * Knudsen number, Prandtl number (must be 1: BGK) and internal degrees of freedom (must be 0). */
@@ -89,12 +89,12 @@ double ugks_mu_ref(const ugks_ctx *);
 long ugks_step_count(const ugks_ctx *);
 /* Kernels launched by this context since ugks_init (for bench.py's gpu_launches). */
 long ugks_launch_count(const ugks_ctx *);
-/* Tuning knobs: name in {"strip" (faces/cells per CTA march), "chunk_m" (velocity rows per chunk), "R" (velocity
- * rows processed in parallel by a CTA), "profile" (1: time every kernel of ugks_step with CUDA events)}.
+/* Tuning knobs: name in {"strip" (cells per CTA march), "chunk_m" (at most that many velocity rows per chunk), "R"
+ * (velocity rows processed in parallel by a CTA), "profile" (1: time every kernel of ugks_step with CUDA events)}.
  * UGKS_EINVAL for unknown names or values that do not fit shared memory / the allocated buffers. */
 int ugks_set_option(ugks_ctx *, const char *name, int value);
 /* With option "profile" on: accumulated device time in ms and launch counts of the five kernels of a step since
- * the last call, in launch order: face_moments(x), face_moments(y), face_scalars, cell_scalars, flux_update.
+ * the last call, in launch order: cell_moments, face_scalars, cell_scalars, tables, flux_update.
  * Synchronises the stream and resets the accumulators. */
 int ugks_kernel_times(ugks_ctx *, double ms[5], long counts[5]);
 const char *ugks_last_error(const ugks_ctx *);           /* library-owned string; ctx may be NULL */

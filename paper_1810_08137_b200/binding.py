@@ -160,7 +160,7 @@ class Ugks:
     def set_option(self, name, value):
         self._chk(lib().ugks_set_option(self._h, name.encode(), int(value)))
 
-    KERNELS = ("face_moments_x", "face_moments_y", "face_scalars", "cell_scalars", "flux_update")
+    KERNELS = ("cell_moments", "face_scalars", "cell_scalars", "tables", "flux_update")
 
     def kernel_times(self):
         """{kernel: (total ms, launches)} since the last call (needs set_option("profile", 1))."""

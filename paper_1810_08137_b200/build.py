@@ -33,8 +33,21 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if verbose:
         flags += ["-Xptxas", "-v"]
     tmp = SO + f".tmp{os.getpid()}"
-    cmd = [nvcc, *flags, "-shared", "-o", tmp, *sources()]
-    subprocess.run(cmd, check=True, cwd=CSRC)
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    hdrs = [d for d in _deps() if not d.endswith(".cu")]
+
+    def compile_one(src):                      # one translation unit -> build/<name>.o, skipped when up to date
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        if not force and os.path.exists(obj) and all(os.path.getmtime(d) <= os.path.getmtime(obj) for d in [src, *hdrs]):
+            return obj
+        subprocess.run([nvcc, *flags, "-c", "-o", obj, src], check=True, cwd=CSRC)
+        return obj
+
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=max(1, min(len(sources()), os.cpu_count() or 1))) as ex:
+        objs = list(ex.map(compile_one, sources()))
+    subprocess.run([nvcc, *[f for f in flags if f not in ("-lineinfo",)], "-shared", "-o", tmp, *objs], check=True, cwd=CSRC)
     os.replace(tmp, SO)
     return SO
 

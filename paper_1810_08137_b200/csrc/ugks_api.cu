@@ -15,7 +15,9 @@ struct ugks_ctx {
     long steps, launches;
     int resblocks, nchunk_alloc;
     double *res_dev, *bcprim_dev, *Wf_dev;
-    double *ghost, *wallg, *Wb, *wallG;     // non-const aliases of the P fields
+    double *ghost, *wallg, *Wb, *wallG, *ghostmom;   // non-const aliases of the P fields
+    int4 *chunks_dev;
+    double *vhost;            // host copy of the v nodes (chunking)
     size_t cells;
     int profile;              // option "profile": time every kernel of ugks_step with CUDA events
     cudaEvent_t *ev; int nev, nev_used;
@@ -40,65 +42,128 @@ static int cuda_fail(ugks_ctx *c, cudaError_t e, const char *where)
 
 static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-// launch geometry heuristics: chunk of velocity rows sized for shared memory,
-// R rows in parallel so that blockDim = Nu*R ~ 128..256 threads, strip length for >= ~4 CTAs per SM
-static void choose_geometry(int I, int J, int Nu, int Nv, int *chunk_m, int *R, int *strip)
+// ---------------------------------------------------------------------------------------------
+// Velocity-row chunks: rows are split into runs of equal sign of v (so that the upwind side of a y-face
+// is uniform over a CTA), each run into equal chunks of at most `cm_target` rows; rows with v = 0 and, if the node order makes
+// too many runs, everything, go to "mixed" chunks that select the side per point.  Order: [v < 0][v > 0][mixed].
+constexpr int MAXCHUNK = 4096;
+struct Chunking { int n, nneg, npos, nmix, cmax; int4 c[MAXCHUNK]; };
+
+static void make_chunks(const double *v, int Nv, int Nu, int cm_target, Chunking *C)
 {
-    int cm = 800 / Nu; if (cm < 1) cm = 1;
-    if (cm >= Nv) cm = Nv;
-    else if ((Nu & 1) && (cm & 1)) cm += 1;                 // 16-byte aligned chunk starts for odd Nu
-    // R rows in parallel, NPT = ceil(cm/R) <= 8 points per thread: minimise issue slots (padded threads x NPT),
-    // prefer NPT near 4..5 (amortises the per-face per-thread setup without starving the SM of warps)
-    int rmax = 256 / Nu; if (rmax < 1) rmax = 1; if (rmax > cm) rmax = cm;
-    int best = rmax; long bestcost = -1;
-    for (int r = rmax; r >= 1; --r) {
-        const int npt = (cm + r - 1) / r;
-        if (npt > 8) break;
-        const long threads = ((long)Nu * r + 31) / 32 * 32;
-        const long cost = threads * npt * 16 + (npt < 4 ? (4 - npt) * 64 : (npt - 4) * 8);
-        if (bestcost < 0 || cost < bestcost) { bestcost = cost; best = r; }
+    if (cm_target < 1) cm_target = 1;
+    if ((Nu & 1) && (cm_target & 1) && cm_target > 1) cm_target -= 1;
+    int4 tmp[MAXCHUNK];
+    int nt = 0, nruns = 0;
+    bool fallback = false;
+    for (int m = 0; m < Nv && !fallback;) {
+        const int sg = v[m] > 0.0 ? 1 : (v[m] < 0.0 ? -1 : 0);
+        int e = m + 1;
+        while (e < Nv && (v[e] > 0.0 ? 1 : (v[e] < 0.0 ? -1 : 0)) == sg) ++e;
+        const int len = e - m, parts = (len + cm_target - 1) / cm_target, rows = (len + parts - 1) / parts;
+        for (int p0 = m; p0 < e; p0 += rows) {
+            if (nt >= MAXCHUNK) { fallback = true; break; }
+            tmp[nt++] = make_int4(p0, (p0 + rows <= e ? rows : e - p0), sg, 0);
+        }
+        m = e;
+        if (++nruns > 8) fallback = true;                            // unsorted nodes: do not shred the grid
     }
-    *chunk_m = cm; *R = best;
-    const int nchunk = (Nv + cm - 1) / cm;
+    if (fallback) {
+        nt = 0;
+        for (int m = 0; m < Nv; m += cm_target) tmp[nt++] = make_int4(m, (m + cm_target <= Nv ? cm_target : Nv - m), 0, 0);
+    }
+    C->n = 0; C->cmax = 0;
+    const int order[3] = { -1, 1, 0 };
+    int cnt[3] = { 0, 0, 0 };
+    for (int o = 0; o < 3; ++o)
+        for (int i = 0; i < nt; ++i)
+            if (tmp[i].z == order[o]) { C->c[C->n++] = tmp[i]; cnt[o]++; if (tmp[i].y > C->cmax) C->cmax = tmp[i].y; }
+    C->nneg = cnt[0]; C->npos = cnt[1]; C->nmix = cnt[2];
+}
+
+// R rows in parallel (threads = Nu*R rounded up to a warp multiple), NPT = ceil(cmax / R) <= 7 points per thread:
+// maximise lane use x point-slot use; ties go to the larger NPT (per-face per-thread setup is amortised over NPT points)
+static void choose_R(int Nu, int cmax, int *R, int *npt)
+{
+    int best = 1; double bestscore = -1.0;
+    for (int r = 1; r <= cmax && Nu * r <= 256; ++r) {
+        const int n = (cmax + r - 1) / r;
+        if (n > 7) continue;
+        const int T = (Nu * r + 31) / 32 * 32;
+        const double score = ((double)Nu * r / T) * ((double)cmax / (r * n));
+        if (score > bestscore + 1e-9) { bestscore = score; best = r; }
+    }
+    *R = best; *npt = (cmax + best - 1) / best;
+}
+
+static void choose_geometry(const double *v, int I, int J, int Nu, int Nv, Chunking *C, int *R, int *npt, int *strip)
+{
+    int cm = 800 / Nu; if (cm < 1) cm = 1; if (cm > 56) cm = 56;
+    make_chunks(v, Nv, Nu, cm, C);
+    choose_R(Nu, C->cmax, R, npt);
     int s = 32;
-    while (s > 8 && (long)J * ((I + s - 1) / s) * nchunk < 148L * 4) s >>= 1;
+    while (s > 8 && (long)J * ((I + s - 1) / s) * C->n < 148L * 4) s >>= 1;
     *strip = s;
 }
 
 struct Layout {
-    size_t f[2], W[2], mom[2], coef[2], fw[2], cellc, respart, res, status, u, wu, v, wv, ghost, wallg, Wb, wallG,
-        bcprim, Wf, total;
-    int Npad, resblocks, nchunk_alloc;
+    size_t f[2], W[2], cmom, frec[2], fw[2], crec, respart, res, status, u, wu, v, wv, ghost, wallg, Wb, wallG, ghostmom,
+        chunks, bcprim, Wf, total;
+    int Npad, resblocks, NuP, NvP, frs, crs, nchunk_alloc;
 };
 static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
 {
-    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > 1024 || vg->Nv < 1) return 1;
+    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > 256 || vg->Nv < 1) return 1;
     const size_t cells = (size_t)m->I * m->J, N = (size_t)vg->Nu * vg->Nv;
     const size_t Npad = (N + 15) & ~(size_t)15;
     const size_t nfx = (size_t)(m->I + 1) * m->J, nfy = (size_t)m->I * (m->J + 1);
-    int cm, R, strip;
-    choose_geometry(m->I, m->J, vg->Nu, vg->Nv, &cm, &R, &strip);
-    const int nchunk = (vg->Nv + cm - 1) / cm;
-    L->nchunk_alloc = nchunk * 2;
+    L->NuP = (vg->Nu + 1) & ~1; L->NvP = (vg->Nv + 1) & ~1;
+    L->frs = FR_NCOEF + L->NuP + L->NvP; L->crs = CR_NCOEF + 2 * L->NuP + 2 * L->NvP;
+    // the moment buffer holds twice the chunks of the default geometry (room for the "chunk_m" tuning option)
+    if (!vg->v) return 1;
+    static Chunking C;
+    int R, npt, strip;
+    choose_geometry(vg->v, m->I, m->J, vg->Nu, vg->Nv, &C, &R, &npt, &strip);
+    size_t nchunk = 2 * (size_t)C.n;
+    if (nchunk > MAXCHUNK) nchunk = MAXCHUNK;
+    L->nchunk_alloc = (int)nchunk;
     L->Npad = (int)Npad;
     L->resblocks = (int)((cells + 127) / 128);
     size_t o = 0;
 #define TAKE(field, bytes) do { L->field = o; o += al256(bytes); } while (0)
     TAKE(f[0], cells * Npad * 8); TAKE(f[1], cells * Npad * 8);
     TAKE(W[0], cells * 32); TAKE(W[1], cells * 32);
-    TAKE(mom[0], nfx * L->nchunk_alloc * NMOM * 8); TAKE(mom[1], nfy * L->nchunk_alloc * NMOM * 8);
-    TAKE(coef[0], nfx * NCOEF * 8); TAKE(coef[1], nfy * NCOEF * 8);
+    TAKE(cmom, cells * nchunk * CMS * 8);
+    TAKE(frec[0], nfx * L->frs * 8); TAKE(frec[1], nfy * L->frs * 8);
     TAKE(fw[0], nfx * 32); TAKE(fw[1], nfy * 32);
-    TAKE(cellc, cells * NCELL * 8);
+    TAKE(crec, cells * L->crs * 8);
     TAKE(respart, (size_t)L->resblocks * 64);
     TAKE(res, 64); TAKE(status, 64);
     TAKE(u, vg->Nu * 8); TAKE(wu, vg->Nu * 8); TAKE(v, vg->Nv * 8); TAKE(wv, vg->Nv * 8);
     TAKE(ghost, 4 * Npad * 8); TAKE(wallg, 4 * Npad * 8);
-    TAKE(Wb, 128); TAKE(wallG, 128); TAKE(bcprim, 128);
+    TAKE(Wb, 128); TAKE(wallG, 128); TAKE(ghostmom, 4 * NRAW * 8); TAKE(bcprim, 128);
+    TAKE(chunks, (size_t)MAXCHUNK * sizeof(int4));
     TAKE(Wf, cells * 32);
 #undef TAKE
     L->total = o;
     return 0;
+}
+
+// install a chunking + (R, npt) in the context: checks buffers and shared memory, uploads the chunk table
+static int apply_geometry(ugks_ctx *c, const Chunking *C, int R, int npt, int nchunk_alloc)
+{
+    UgksParams T = c->P;
+    T.nchunk = C->n; T.nneg = C->nneg; T.npos = C->npos; T.nmix = C->nmix; T.cmax = C->cmax; T.R = R; T.npt = npt;
+    if (C->n > nchunk_alloc) return fail(c, UGKS_EINVAL, "%s", "too many chunks for the allocated moment buffer");
+    if (npt < 1 || npt > 7 || R < 1 || T.Nu * R > 256 || R * npt < C->cmax) return fail(c, UGKS_EINVAL, "%s", "R / points per thread out of range");
+    if (smem_flux_update(T) > 227 * 1024 || smem_cell_moments(T) > 227 * 1024) return fail(c, UGKS_EINVAL, "%s", "chunk does not fit in shared memory");
+    for (int i = 0; i < C->n; ++i)
+        if ((T.Nu & 1) && (C->c[i].x & 1) && 0) return fail(c, UGKS_EINVAL, "%s", "unaligned chunk");
+    CK(cudaStreamSynchronize(c->st), "apply_geometry");
+    CK(cudaMemcpy(c->chunks_dev, C->c, sizeof(int4) * C->n, cudaMemcpyHostToDevice), "apply_geometry");
+    c->P = T;
+    if (setup_moments_attributes(c->P) || setup_update_attributes(c->P)) return cuda_fail(c, cudaGetLastError(), "apply_geometry");
+    return UGKS_OK;
 }
 
 extern "C" {
@@ -120,7 +185,7 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     *out = nullptr;
     if (!m || !vg || !gas || !bcs || !workspace_dev) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     Layout L;
-    if (make_layout(m, vg, &L)) return fail(c, UGKS_EINVAL, "%s", "invalid mesh or velocity grid size (I,J >= 2; 1 <= Nu <= 1024)");
+    if (make_layout(m, vg, &L)) return fail(c, UGKS_EINVAL, "%s", "invalid mesh or velocity grid size (I,J >= 2; 1 <= Nu <= 256)");
     if (!(m->x1 > m->x0) || !(m->y1 > m->y0)) return fail(c, UGKS_EINVAL, "%s", "empty domain");
     if (!vg->u || !vg->wu || !vg->v || !vg->wv) return fail(c, UGKS_EINVAL, "%s", "NULL velocity arrays");
     if (gas->Pr != 1.0) return fail(c, UGKS_EINVAL, "%s", "Pr must be 1 (BGK)");
@@ -164,19 +229,24 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     char *base = (char *)workspace_dev;
     auto D = [&](size_t off) { return (double *)(base + off); };
     P.f[0] = D(L.f[0]); P.f[1] = D(L.f[1]); P.W[0] = D(L.W[0]); P.W[1] = D(L.W[1]);
-    P.mom[0] = D(L.mom[0]); P.mom[1] = D(L.mom[1]); P.coef[0] = D(L.coef[0]); P.coef[1] = D(L.coef[1]);
-    P.fw[0] = D(L.fw[0]); P.fw[1] = D(L.fw[1]); P.cellc = D(L.cellc); P.respart = D(L.respart);
+    P.cmom = D(L.cmom); P.frec[0] = D(L.frec[0]); P.frec[1] = D(L.frec[1]);
+    P.fw[0] = D(L.fw[0]); P.fw[1] = D(L.fw[1]); P.crec = D(L.crec); P.respart = D(L.respart);
+    P.NuP = L.NuP; P.NvP = L.NvP; P.frs = L.frs; P.crs = L.crs;
     P.status = (int *)(base + L.status);
     P.u = D(L.u); P.wu = D(L.wu); P.v = D(L.v); P.wv = D(L.wv);
-    c->ghost = D(L.ghost); c->wallg = D(L.wallg); c->Wb = D(L.Wb); c->wallG = D(L.wallG);
-    P.ghost = c->ghost; P.wallg = c->wallg; P.Wb = c->Wb; P.wallG = c->wallG;
+    c->ghost = D(L.ghost); c->wallg = D(L.wallg); c->Wb = D(L.Wb); c->wallG = D(L.wallG); c->ghostmom = D(L.ghostmom);
+    P.ghost = c->ghost; P.wallg = c->wallg; P.Wb = c->Wb; P.wallG = c->wallG; P.ghostmom = c->ghostmom;
+    c->chunks_dev = (int4 *)(base + L.chunks); P.chunks = c->chunks_dev;
     c->res_dev = D(L.res); c->bcprim_dev = D(L.bcprim); c->Wf_dev = D(L.Wf);
     c->resblocks = L.resblocks; c->nchunk_alloc = L.nchunk_alloc;
+    c->vhost = (double *)malloc(sizeof(double) * vg->Nv);
+    if (!c->vhost) { free(c); return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed"); }
+    memcpy(c->vhost, vg->v, sizeof(double) * vg->Nv);
     c->cells = (size_t)m->I * m->J;
     c->st = (cudaStream_t)cuda_stream;
-    choose_geometry(P.I, P.J, P.Nu, P.Nv, &P.chunk_m, &P.R, &P.strip);
-    P.nchunk = (P.Nv + P.chunk_m - 1) / P.chunk_m;
-    P.npt = (P.chunk_m + P.R - 1) / P.R;
+    static Chunking C;
+    int R0, npt0;
+    choose_geometry(vg->v, P.I, P.J, P.Nu, P.Nv, &C, &R0, &npt0, &P.strip);
 
     double bcprim[16];
     for (int s = 0; s < 4; ++s) { bcprim[s * 4] = b[s]->rho; bcprim[s * 4 + 1] = b[s]->U; bcprim[s * 4 + 2] = b[s]->V; bcprim[s * 4 + 3] = b[s]->T; }
@@ -188,10 +258,15 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     if (e == cudaSuccess) e = cudaMemsetAsync(P.f[0], 0, c->cells * P.Npad * 8, c->st);
     if (e == cudaSuccess) e = cudaMemsetAsync(P.f[1], 0, c->cells * P.Npad * 8, c->st);
     if (e == cudaSuccess) e = cudaMemsetAsync(P.status, 0, 64, c->st);
-    if (e == cudaSuccess) { c->launches += launch_setup(P, c->bcprim_dev, c->ghost, c->wallg, c->Wb, c->wallG, c->st); e = cudaGetLastError(); }
-    if (e == cudaSuccess && (setup_moments_attributes(P) || setup_update_attributes(P))) e = cudaGetLastError() == cudaSuccess ? cudaErrorInvalidValue : cudaErrorInvalidValue;
+    if (e == cudaSuccess) e = cudaMemsetAsync(P.cmom, 0, c->cells * (size_t)L.nchunk_alloc * CMS * 8, c->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(P.frec[0], 0, (size_t)nfaces_x(P) * P.frs * 8, c->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(P.frec[1], 0, (size_t)nfaces_y(P) * P.frs * 8, c->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(P.crec, 0, c->cells * (size_t)P.crs * 8, c->st);
+    if (e == cudaSuccess) { c->launches += launch_setup(P, c->bcprim_dev, c->ghost, c->wallg, c->Wb, c->wallG, c->ghostmom, c->st); e = cudaGetLastError(); }
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
-    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); free(c); return rc; }
+    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); free(c->vhost); free(c); return rc; }
+    { const int rc = apply_geometry(c, &C, R0, npt0, c->nchunk_alloc);
+      if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); free(c->vhost); free(c); return rc; } }
     *out = c;
     return UGKS_OK;
 }
@@ -202,6 +277,7 @@ void ugks_destroy(ugks_ctx *c)
     cudaStreamSynchronize(c->st);
     for (int i = 0; i < c->nev; ++i) cudaEventDestroy(c->ev[i]);
     free(c->ev);
+    free(c->vhost);
     free(c);
 }
 
@@ -219,19 +295,21 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
         P.strip = value;
         return UGKS_OK;
     }
-    if (!strcmp(name, "chunk_m") || !strcmp(name, "R")) {
-        int cm = P.chunk_m, R = P.R;
-        if (!strcmp(name, "chunk_m")) cm = value; else R = value;
-        if (cm < 1 || cm > P.Nv || R < 1 || P.Nu * R > 1024) return fail(c, UGKS_EINVAL, "%s", "chunk_m / R out of range");
-        const int nchunk = (P.Nv + cm - 1) / cm;
-        if (nchunk > c->nchunk_alloc) return fail(c, UGKS_EINVAL, "%s", "chunk_m too small for the allocated moment buffers");
-        if (nchunk > 1 && ((cm * P.Nu) & 1)) return fail(c, UGKS_EINVAL, "%s", "chunk_m * Nu must be even (16-byte aligned chunks)");
-        UgksParams T = P; T.chunk_m = cm; T.R = R; T.nchunk = nchunk; T.npt = (cm + R - 1) / R;
-        if (T.npt > 8) return fail(c, UGKS_EINVAL, "%s", "chunk_m / R must be <= 8 points per thread");
-        if (smem_flux_update(T) > 227 * 1024) return fail(c, UGKS_EINVAL, "%s", "chunk does not fit in shared memory");
-        P = T;
-        if (setup_moments_attributes(P) || setup_update_attributes(P)) return cuda_fail(c, cudaGetLastError(), "ugks_set_option");
-        return UGKS_OK;
+    if (!strcmp(name, "chunk_m")) {                                  // re-chunk with at most `value` rows per chunk
+        if (value < 1 || value > 56) return fail(c, UGKS_EINVAL, "%s", "chunk_m out of range");
+        static Chunking C;
+        make_chunks(c->vhost, P.Nv, P.Nu, value, &C);
+        int R, npt;
+        choose_R(P.Nu, C.cmax, &R, &npt);
+        return apply_geometry(c, &C, R, npt, c->nchunk_alloc);
+    }
+    if (!strcmp(name, "R")) {
+        if (value < 1 || P.Nu * value > 256) return fail(c, UGKS_EINVAL, "%s", "R out of range");
+        static Chunking C;
+        CK(cudaStreamSynchronize(c->st), "ugks_set_option");
+        CK(cudaMemcpy(C.c, c->chunks_dev, sizeof(int4) * P.nchunk, cudaMemcpyDeviceToHost), "ugks_set_option");
+        C.n = P.nchunk; C.nneg = P.nneg; C.npos = P.npos; C.nmix = P.nmix; C.cmax = P.cmax;
+        return apply_geometry(c, &C, value, (P.cmax + value - 1) / value, c->nchunk_alloc);
     }
     if (!strcmp(name, "profile")) { c->profile = value != 0; return UGKS_OK; }
     return fail(c, UGKS_EINVAL, "unknown option %s", name);
@@ -278,15 +356,15 @@ int ugks_step(ugks_ctx *c, int n)
     for (int s = 0; s < n; ++s) {
         cudaEvent_t *e = c->profile ? c->ev + c->nev_used : nullptr;
         if (e) cudaEventRecord(e[0], c->st);
-        c->launches += launch_face_moments(c->P, c->cur, 0, c->st);    // R, S1, S7 sums, x-faces
+        c->launches += launch_cell_moments(c->P, c->cur, c->st);       // R, S1, S7 sums (both directions)
         if (e) cudaEventRecord(e[1], c->st);
-        c->launches += launch_face_moments(c->P, c->cur, 1, c->st);    // ... y-faces
-        if (e) cudaEventRecord(e[2], c->st);
         c->launches += launch_face_scalars(c->P, c->cur, c->st);       // S2..S5, wall density
+        if (e) cudaEventRecord(e[2], c->st);
+        c->launches += launch_cell_scalars(c->P, c->cur, c->resblocks, c->st);   // U1, U2 scalars, residual partials
         if (e) cudaEventRecord(e[3], c->st);
-        c->launches += launch_cell_scalars(c->P, c->cur, c->resblocks, c->st);   // U1, U2, residual partials
+        c->launches += launch_tables(c->P, c->st);                     // S6 / U2 separable Maxwellian factors
         if (e) cudaEventRecord(e[4], c->st);
-        c->launches += launch_flux_update(c->P, c->cur, c->st);        // S6, S8, U3
+        c->launches += launch_flux_update(c->P, c->cur, c->st);        // R, S6, S8, U3
         if (e) { cudaEventRecord(e[5], c->st); c->nev_used += 6; }
         c->cur ^= 1;
         c->steps += 1;

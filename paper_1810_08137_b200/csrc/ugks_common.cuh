@@ -9,22 +9,38 @@
 
 enum { BC_PERIODIC = 0, BC_FIXED = 1, BC_WALL = 2 };
 
-constexpr int NMOM = 12;    // per-(face,chunk) raw moments: 11 used, padded to 12
-constexpr int NCOEF = 24;   // per-face coefficients consumed by the flux/update kernel
-constexpr int NCELL = 12;   // per-cell coefficients consumed by the flux/update kernel
-constexpr int RINGX = 6;    // face_moments: stencil ring slots (4 live rows + 2 in flight)
-constexpr int NSX = 4;      // flux_update: x-ring slots (2 live rows + 2 in flight; older rows live in registers)
+// ---------------------------------------------------------------------------------------------
+// Per-(cell, chunk) half-range moment sets written by k_cell_moments and summed per face by k_face_scalars.
+// A cell contributes (f_c + h sigma_c) to its plus-side face where n > 0 and (f_c - h sigma_c) to its minus-side face
+// where n < 0 (O3 written cell by cell); sets: 0 = x+, 1 = x-, 2 = y+, 3 = y-.  13 raw sums per set, local frame,
+// M_ab = sum w n^a t^b f0, S_ab = sum w n^a t^b (h sigma0):
+constexpr int NSET = 4, NRAW = 13, CMS = NSET * NRAW;
+enum { RW_M00 = 0, RW_M10, RW_M20, RW_M30, RW_M01, RW_M11, RW_M02, RW_M12, RW_S20, RW_S30, RW_S40, RW_S21, RW_S22 };
 
-// coefficient record written by k_face_scalars (S2..S5) and read by k_flux_update (S6, S8)
-// P(n,t) = Mt1 + Mt2 (n a.psi + t b.psi) + Mt3 A.psi = sum c_ab n^a t^b (total degree <= 3); the five coefficients that
-// contain a (c10, c20, c30, c11, c12) come in an L (n > 0, a_L) and an R (n < 0, a_R) variant.
-enum { CF_C0 = 0, CF_U = 1, CF_V = 2, CF_LAM = 3, CF_MT4 = 4, CF_MT5 = 5, CF_RHOW = 6, CF_TYPE = 7,
-       CF_C00 = 8, CF_C01 = 9, CF_C02 = 10, CF_C03 = 11, CF_C21 = 12, CF_L = 13, CF_R = 18 };
-// per-cell record written by k_cell_scalars (U1, U2) and read by k_flux_update (U3)
-enum { CC_GN = 0, CC_UN = 1, CC_VN = 2, CC_LN = 3, CC_GP = 4, CC_UP = 5, CC_VP = 6, CC_LP = 7, CC_KF = 8, CC_KD = 9 };
+// Face record written by k_face_scalars (S2..S5; 24 coefficients) and k_tables (separable Maxwellian factors):
+//   [0, FR_NCOEF)                        coefficients, see FR_*
+//   [FR_NCOEF, FR_NCOEF + NuP)           E_k[k] = exp(-lam (u_k - c_u)^2)   (c_u = U0 on x-faces, V0 (tangential) on y-faces)
+//   [FR_NCOEF + NuP, FR_NCOEF + NuP+NvP) E_m[m] = exp(-lam (v_m - c_v)^2)
+// Flux polynomial  ell C0 [Mt1 + Mt2 (n a.psi + t b.psi) + Mt3 A.psi] = sum c_ab n^a t^b (total degree <= 3); the five
+// coefficients that contain a (c10, c20, c30, c11, c12) come in an L (n > 0, a_L) and an R (n < 0, a_R) variant.
+constexpr int FR_NCOEF = 24;
+enum { FR_LAM = 0, FR_U = 1, FR_V = 2, FR_TYPE = 3, FR_RHOW = 4, FR_MT4 = 5 /* ell Mt4 */, FR_MT5 = 6 /* -ell Mt5 2/Delta */,
+       FR_TAU = 7, FR_C00 = 8, FR_C01 = 9, FR_C02 = 10, FR_C03 = 11, FR_C21 = 12, FR_L = 13, FR_R = 18 };
+// offsets inside FR_L / FR_R
+enum { LR_C10 = 0, LR_C20 = 1, LR_C30 = 2, LR_C11 = 3, LR_C12 = 4 };
+
+// Cell record written by k_cell_scalars (U1, U2 scalars) and k_tables:
+//   [0, CR_NCOEF)                          see CR_*
+//   [CR_NCOEF, +NuP)                       gn_u[k] = GN exp(-lam_n (u_k - U_n)^2)    (relaxation prefactors folded in)
+//   [CR_NCOEF + NuP, +NuP)                 gp_u[k] = GP exp(-lam_p (u_k - U_p)^2)
+//   [CR_NCOEF + 2 NuP, +2 Nv)              pairs (gn_v[m], gp_v[m]) = (exp(-lam_n (v_m - V_n)^2), exp(-lam_p (v_m - V_p)^2))
+constexpr int CR_NCOEF = 12;
+enum { CR_KF = 0, CR_KD = 1, CR_GN = 2, CR_GP = 3, CR_UN = 4, CR_VN = 5, CR_LN = 6, CR_UP = 7, CR_VP = 8, CR_LP = 9 };
 
 struct UgksParams {
     int I, J, Nu, Nv, N, Npad;
+    int NuP, NvP;                    // Nu, Nv rounded up to even (16-byte aligned table segments)
+    int frs, crs;                    // record strides in doubles: FR_NCOEF + NuP + NvP, CR_NCOEF + 2 NuP + 2 NvP
     double dx, dy, dt, omega, mu_ref;
     int bc[4];                       // xmin, xmax, ymin, ymax
     const double *u, *wu, *v, *wv;   // device copies of the velocity nodes / weights
@@ -32,45 +48,55 @@ struct UgksParams {
     const double *wallg;             // [4][Npad] wall Maxwellians of (1,Uw,Vw,1/Tw) (O0)
     const double *Wb;                // [4][4]   cons(prim_b) of FIXED sides
     const double *wallG;             // [4][4]   sum_{outgoing} w n psi_loc g_w per wall side (local frame)
+    const double *ghostmom;          // [4][NRAW] half-range raw moments of the ghost row toward the domain (FIXED sides)
+    const int4 *chunks;              // [nchunk] (m0, mc, sign of v over the chunk: +1 / -1 / 0 = mixed, 0)
     double *f[2];                    // ping-pong copies of f, rows padded to Npad
     double *W[2];                    // ping-pong copies of W [cells][4]
-    double *mom[2];                  // [faces][nchunk][NMOM], x then y faces
-    double *coef[2];                 // [faces][NCOEF]
+    double *cmom;                    // [cells][nchunk][NSET][NRAW]
+    double *frec[2];                 // [faces][frs], x then y faces
     double *fw[2];                   // [faces][4] time-integrated macroscopic flux, global frame
-    double *cellc;                   // [cells][NCELL]
+    double *crec;                    // [cells][crs]
     double *respart;                 // [resblocks][8] partial residual sums
     int *status;                     // [2]: non-physical-state flags
-    int strip;                       // faces / cells per CTA march
-    int chunk_m;                     // velocity rows (m) per chunk
-    int nchunk;                      // chunks per row of f
-    int R;                           // m-rows processed in parallel by one CTA (blockDim = Nu*R)
-    int npt;                         // velocity points per thread = ceil(chunk_m / R), 1..8 (template parameter)
+    int strip;                       // cells per CTA march
+    int nchunk;                      // velocity-row chunks (sign-uniform where possible), sorted [v < 0][v > 0][mixed]
+    int nneg, npos, nmix;            // chunks per class
+    int cmax;                        // rows of the largest chunk
+    int R;                           // velocity rows processed in parallel by one CTA (threads = Nu*R rounded up to 32)
+    int npt;                         // velocity points per thread = ceil(cmax / R), 1..8 (template parameter)
 };
 
 static __host__ __device__ inline int nfaces_x(const UgksParams &P) { return (P.I + 1) * P.J; }
 static __host__ __device__ inline int nfaces_y(const UgksParams &P) { return P.I * (P.J + 1); }
+static __host__ __device__ inline int pad2(int x) { return (x + 1) & ~1; }
 
 // ---------------------------------------------------------------------------------------------
 // row lookup (O1): returns the row of cell `pos` on the line (dir 0: (pos,line), dir 1: (line,pos)),
-// resolving PERIODIC wrap and FIXED ghosts.  A WALL neighbour is "missing": *missing = 1 and a valid
-// (clamped) row is returned so that staging stays uniform; its values are never used.
+// resolving PERIODIC wrap and FIXED ghosts.  A WALL neighbour is "missing": a valid (clamped) row is returned so
+// that staging stays uniform; its values are never used.
 template <int DIR>
-__device__ __forceinline__ const double *row_ptr(const UgksParams &P, const double *f, int pos, int line, int *missing)
+__device__ __forceinline__ const double *row_ptr(const UgksParams &P, const double *f, int pos, int line)
 {
     const int n = DIR == 0 ? P.I : P.J;
     const int lo = DIR == 0 ? 0 : 2, hi = lo + 1;
-    *missing = 0;
     if (pos < 0) {
         if (P.bc[lo] == BC_PERIODIC) pos += n;
         else if (P.bc[lo] == BC_FIXED) return P.ghost + (size_t)lo * P.Npad;
-        else { *missing = 1; pos = 0; }
+        else pos = 0;
     } else if (pos >= n) {
         if (P.bc[hi] == BC_PERIODIC) pos -= n;
         else if (P.bc[hi] == BC_FIXED) return P.ghost + (size_t)hi * P.Npad;
-        else { *missing = 1; pos = n - 1; }
+        else pos = n - 1;
     }
     const size_t cell = DIR == 0 ? (size_t)line * P.I + pos : (size_t)pos * P.I + line;
     return f + cell * P.Npad;
+}
+// is cell `pos` of a line beyond a WALL side?
+template <int DIR>
+__device__ __forceinline__ bool beyond_wall(const UgksParams &P, int pos)
+{
+    const int n = DIR == 0 ? P.I : P.J, lo = DIR == 0 ? 0 : 2;
+    return (pos < 0 && P.bc[lo] == BC_WALL) || (pos >= n && P.bc[lo + 1] == BC_WALL);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -98,12 +124,21 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 }
 
 // ---------------------------------------------------------------------------------------------
-// h*sigma of the van Leer limiter (AMB-4) from un-normalised differences dm = f_c - f_{c-1},
-// dp = f_{c+1} - f_c:  h*sigma = (dx/2) * 2 (dm/dx)(dp/dx)/((dm+dp)/dx) = dm dp / (dm + dp).
+// h*sigma of the van Leer limiter (AMB-4) from un-normalised differences dm = f_c - f_{c-1}, dp = f_{c+1} - f_c:
+//   h*sigma = (Delta/2) * 2 (dm/Delta)(dp/Delta)/((dm+dp)/Delta) = dm dp / (dm + dp)   if dm dp > 0, else 0.
+// The reciprocal is MUFU.RCP64H (rel. error 2^-23) refined by one cubic step r (1 + e + e^2), e = 1 - s r: error
+// e^3 ~ 2^-69, i.e. r is within ~1 ulp.  When dm dp > 0 (as a normal double) the sum is a normal number.  The sign test reads
+// the high word: a product that underflowed to a denormal counts as 0, as in AMB-4's "underflow gives sigma = 0".
 __device__ __forceinline__ double vl_half(double dm, double dp)
 {
-    const double pr = dm * dp;
-    return pr > 0.0 ? pr / (dm + dp) : 0.0;
+    const double pr = dm * dp, s = dm + dp;
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));
+    const double e = fma(-s, r, 1.0);
+    const double t = fma(e, e, e);
+    r = fma(r, t, r);
+    const double hs = pr * r;
+    return __double2hiint(pr) > 0 ? hs : 0.0;
 }
 
 __device__ __forceinline__ double warp_sum(double x)
@@ -114,15 +149,16 @@ __device__ __forceinline__ double warp_sum(double x)
 }
 
 // launchers (one per translation unit); each returns the number of kernels it enqueued
-int launch_face_moments(const UgksParams &P, int cur, int dir, cudaStream_t st);
+int launch_cell_moments(const UgksParams &P, int cur, cudaStream_t st);
 int launch_face_scalars(const UgksParams &P, int cur, cudaStream_t st);
 int launch_cell_scalars(const UgksParams &P, int cur, int resblocks, cudaStream_t st);
+int launch_tables(const UgksParams &P, cudaStream_t st);
 int launch_flux_update(const UgksParams &P, int cur, cudaStream_t st);
 int launch_setup(const UgksParams &P, const double *bc_prims /*dev [4][4]*/, double *ghost, double *wallg,
-                 double *Wb, double *wallG, cudaStream_t st);
+                 double *Wb, double *wallG, double *ghostmom, cudaStream_t st);
 int launch_residual_final(const UgksParams &P, int resblocks, double *res_dev, cudaStream_t st);
 int launch_moments_of_f(const UgksParams &P, const double *f, double *Wf, cudaStream_t st);
 int setup_moments_attributes(const UgksParams &P);
 int setup_update_attributes(const UgksParams &P);
-size_t smem_face_moments(const UgksParams &P);
+size_t smem_cell_moments(const UgksParams &P);
 size_t smem_flux_update(const UgksParams &P);

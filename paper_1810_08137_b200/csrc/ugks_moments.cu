@@ -1,313 +1,308 @@
-// ugks_moments.cu -- k_face_moments: reconstruction (R) and the velocity-space reductions of S1 and S7
-// ("12 times parallel reduction") for every cell face.
+// ugks_moments.cu -- k_cell_moments: reconstruction (R) and the velocity-space reductions of S1 and S7
+// ("12 times parallel reduction"), written cell by cell.
 //
-// One CTA marches along a strip of consecutive faces of one grid line (x-faces of row j, or y-faces of column i)
-// for one chunk of velocity rows.  Thread (k, r) owns velocity column k and the NPT rows m = r + p*R.
-//   * stencil: each thread keeps its two upwind-side rows in registers and reads ONE new row per face from a
-//     4-slot shared-memory ring fed by 1-D TMA bulk copies (cp.async.bulk + mbarrier), two rows in flight.
-//   * the 11 distinct moments of f0 and sigma0 are tensor products: per thread only sum_m wv v^p (.) is
-//     accumulated (6-7 sums); the reduction is a three-stage pipeline across consecutive faces, one stage per
-//     face step and no extra barrier: (1) partial sums to shared memory, (2) sum over the R threads of each
-//     column k, (3) one warp applies the k-dependent factors wu u^a once per column and finishes with a
-//     transposing shuffle butterfly (16 shuffles for 16 values instead of 5 per value).
+// The upwind face state of O3 is f0 = f_c + h sigma_c on the plus-side face of cell c where n > 0 and f_c - h sigma_c on
+// its minus-side face where n < 0, so every face sum splits into a part owned by the left cell and a part owned by the
+// right cell.  One pass over the cells therefore serves the x- and the y-faces: per cell and direction ONE limiter
+// evaluation per velocity point, from the centred stencil (c-1, c, c+1), and f is read from HBM once.
+//
+// One CTA marches along a strip of cells of row j for one chunk of velocity rows (all v_m of one sign where the grid
+// allows, so that the y-side of a point is CTA-uniform).  Thread (k, r) owns velocity column k and the rows m = r + p*R.
+//   * x-stencil: (f_c, f_c - f_{c-1}) live in registers; ONE new row per cell comes from a 3-slot shared-memory ring fed by
+//     1-D TMA bulk copies (cp.async.bulk + mbarrier).  y-neighbours (i, j-1), (i, j+1): TMA-staged, double-buffered.
+//   * sums are tensor products: a thread accumulates sum_m wv v^p (.) for its column (13 sums; weights wv v^p come as
+//     broadcast shared-memory loads); three pipelined stages, one per cell step, finish the reduction without an extra
+//     barrier: (1) partial sums to shared memory, (2) sum over the R threads of a column, (3) per output one thread (or
+//     2 / 4) takes the dot product over k with the factors wu u^a H(+-u).
 #include "ugks_common.cuh"
 #include <type_traits>
 
-constexpr int NACC = 7;
-constexpr int NSM = 4;       // stencil ring slots: 2 live rows + 2 in flight (8 slots measured no faster: not latency-bound)
+constexpr int NSXM = 3;                                              // x-ring slots
+constexpr int NFAC = 13;                                             // factor tables: 5 (x+), 5 (x-), 3 (y)
+__constant__ int c_xa[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 2, 3, 4, 2, 2 };   // power of n = u_k of raw sum idx (x sets)
+__constant__ int c_xc[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 3, 3, 3, 4, 5 };   // column sum: 0..2 = C_b (+- B_b), 3..5 = B_b
+__constant__ int c_yt[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 0, 0, 0, 1, 2 };   // power of t = u_k (y sets)
+__constant__ int c_yc[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 4, 5, 6, 4, 4 };   // column sum: A_0..A_3, B_2..B_4
 
-__device__ __forceinline__ double vl_half_rcp(double dm, double dp)
+template <int NPT, bool MIXED, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P, const int cur, const int chunk0)
 {
-    const double pr = dm * dp, s = dm + dp;
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));
-    double e = fma(-s, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-s, r, 1.0);
-    r = fma(r, e, r);
-    return pr > 0.0 ? pr * r : 0.0;
-}
-
-// upwind state at the face for the moment sums: f0 = f_c + sg * h sigma_c, hs = h sigma_c (O3).
-// FL: mm / mp = minus / plus neighbour is a wall (one-sided, AMB-13); mc = the upwind "cell" is the wall itself:
-// nothing comes from the fluid on that side, the face sums take 0 there (the wall part is analytic, O9).
-template <bool FL>
-__device__ __forceinline__ void recon_m(double fm, double fc, double fp, double sg, bool mm, bool mc, bool mp, double &f0, double &hs)
-{
-    double dm = fc - fm, dp = fp - fc;
-    if (FL) { if (mm) dm = dp; if (mp) dp = dm; }
-    hs = vl_half_rcp(dm, dp);
-    f0 = fma(sg, hs, fc);
-    if (FL && mc) { f0 = 0.0; hs = 0.0; }
-}
-
-template <int DIR>
-__device__ __forceinline__ int miss_mask_m(const UgksParams &P, int a)
-{
-    const int n = DIR == 0 ? P.I : P.J, lo = DIR == 0 ? 0 : 2;
-    const bool wlo = P.bc[lo] == BC_WALL, whi = P.bc[lo + 1] == BC_WALL;
-    int ms = 0;
-#pragma unroll
-    for (int d = 0; d < 4; ++d) {
-        const int pos = a - 2 + d;
-        if ((pos < 0 && wlo) || (pos >= n && whi)) ms |= 1 << d;
-    }
-    return ms;
-}
-
-template <int DIR, int NPT, int MAXT, int MINB>
-__global__ void __launch_bounds__(MAXT, MINB) k_face_moments(const UgksParams P, const int cur)
-{
+    constexpr int NA = MIXED ? 20 : 13;                              // column sums per thread: 6 (x) + 7 (y) [+ 7 (y-)]
+    constexpr int NOUT = MIXED ? 4 * NRAW : 3 * NRAW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int nline = DIR == 0 ? P.J : P.I;
-    const int npos = (DIR == 0 ? P.I : P.J) + 1;
-    const int nstrip = (npos + P.strip - 1) / P.strip;
+    const int nstrip = (P.I + P.strip - 1) / P.strip;
     int b = blockIdx.x;
-    const int line = b % nline; b /= nline;
+    const int j = b % P.J; b /= P.J;
     const int s = b % nstrip;
-    const int chunk = b / nstrip;
-    const int a0 = s * P.strip, a1 = min(a0 + P.strip, npos);      // faces [a0, a1)
-    const int m0 = chunk * P.chunk_m, mc = min(P.chunk_m, P.Nv - m0);
-    const int Nu = P.Nu, R = P.R, CM = P.chunk_m, Q = mc * Nu, q0 = m0 * Nu;
-    const int Qs = (CM * Nu + 1) & ~1;
-    const uint32_t bytes = (uint32_t)(((Q + 1) & ~1) * sizeof(double));
+    const int chunk = chunk0 + b / nstrip;                           // chunks are sorted: [v < 0][v > 0][mixed]
+    const int4 ch = P.chunks[chunk];
+    const int c0 = s * P.strip, c1 = min(c0 + P.strip, P.I);         // cells [c0, c1)
+    const int m0 = ch.x, mc = ch.y;
+    const int Nu = P.Nu, R = P.R;
+    const int q0 = m0 * Nu, qa = q0 & ~1, qsh = q0 - qa;             // 16-byte aligned copy start; shift of the chunk inside
+    const int Qb = pad2(P.cmax * Nu + 1);
+    const uint32_t bytes = (uint32_t)(pad2(mc * Nu + qsh) * sizeof(double));
     const int B = blockDim.x;
+    const int nrow = R * NPT + 1;                                    // weight rows incl. a zero row
 
-    double *ring = reinterpret_cast<double *>(smem_raw);            // [NSM][Qs]
-    double *part = ring + (size_t)NSM * Qs;                         // [2][NACC][B]   per-thread partial sums
-    double *col = part + 2 * NACC * B;                              // [2][NACC][Nu]  per-column sums
-    double *un = col + 2 * NACC * Nu;                               // [Nu] u_k, then [Nu] wu_k
-    double *wun = un + Nu;
-    double *vn = wun + Nu;                                          // [CM] v_m, then [CM] wv_m
-    double *wvn = vn + CM;
-    double *red = wvn + CM;                                         // [2][32][16] per-warp moment sums
-    uint64_t *bars = reinterpret_cast<uint64_t *>(red + 2 * 32 * 16);
+    double *xring = reinterpret_cast<double *>(smem_raw);            // [NSXM][Qb]
+    double *ybuf = xring + (size_t)NSXM * Qb;                        // [2][2][Qb]
+    double *part = ybuf + (size_t)4 * Qb;                            // [2][NA][B]
+    double *col = part + (size_t)2 * NA * B;                         // [2][NA][Nu]
+    double *fac = col + (size_t)2 * NA * Nu;                         // [NFAC][Nu]
+    double *mtab = fac + (size_t)pad2(NFAC * Nu);                    // [nrow][6]: w, w v, w v^2, w v^3, w v^4, H(v)
+    int4 *desc = reinterpret_cast<int4 *>(mtab + (size_t)pad2(nrow * 6));      // [NOUT] stage-3 output descriptors
+    uint64_t *bars = reinterpret_cast<uint64_t *>(desc + NOUT);     // [NSXM] x rows, [2] y stages
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = B >> 5;
+    const int tid = threadIdx.x;
     const bool active = tid < Nu * R;
-    const int k = tid % Nu, r = tid / Nu;
+    const int k = active ? tid % Nu : 0, r = active ? tid / Nu : 0;
     const double *fcur = P.f[cur];
-    const int rows_first = a0 - 2, rows_last = a1;                  // cells a0-2 .. a1 are staged
+    const int rows_first = c0 - 1, rows_last = c1;                   // cells c0-1 .. c1 are staged
 
-    auto issue = [&](int row) {
-        int miss;
-        const int sl = (row - rows_first) % NSM;
-        const double *src = row_ptr<DIR>(P, fcur, row, line, &miss) + q0;
+    auto issue_x = [&](int row) {
+        const int sl = (row - rows_first) % NSXM;
+        const double *src = row_ptr<0>(P, fcur, row, j) + qa;
         mbar_expect_tx(&bars[sl], bytes);
-        tma_load_1d(ring + (size_t)sl * Qs, src, bytes, &bars[sl]);
+        tma_load_1d(xring + (size_t)sl * Qb, src, bytes, &bars[sl]);
     };
-    auto wait_row = [&](int row) {
+    auto wait_x = [&](int row) {
         const int idx = row - rows_first;
-        mbar_wait(&bars[idx % NSM], (idx / NSM) & 1);
+        mbar_wait(&bars[idx % NSXM], (idx / NSXM) & 1);
+    };
+    auto issue_y = [&](int cell) {
+        const int buf = (cell - c0) & 1;
+        mbar_expect_tx(&bars[NSXM + buf], 2 * bytes);
+        tma_load_1d(ybuf + (size_t)(buf * 2) * Qb, row_ptr<1>(P, fcur, j - 1, cell) + qa, bytes, &bars[NSXM + buf]);
+        tma_load_1d(ybuf + (size_t)(buf * 2 + 1) * Qb, row_ptr<1>(P, fcur, j + 1, cell) + qa, bytes, &bars[NSXM + buf]);
     };
 
     if (tid == 0) {
-        for (int i = 0; i < NSM; ++i) mbar_init(&bars[i], 1);
+        for (int i = 0; i < NSXM + 2; ++i) mbar_init(&bars[i], 1);
         mbar_fence_init();
     }
-    for (int i = tid; i < Nu; i += B) { un[i] = P.u[i]; wun[i] = P.wu[i]; }
-    for (int i = tid; i < mc; i += B) { vn[i] = P.v[m0 + i]; wvn[i] = P.wv[m0 + i]; }
+    for (int i = tid; i < Nu; i += B) {
+        const double u = P.u[i], w = P.wu[i];
+        const double hp = u > 0.0 ? 1.0 : (u < 0.0 ? 0.0 : 0.5);
+        double pw = 1.0;
+        for (int a = 0; a < 5; ++a) {
+            fac[a * Nu + i] = w * hp * pw;
+            fac[(5 + a) * Nu + i] = w * (1.0 - hp) * pw;
+            if (a < 3) fac[(10 + a) * Nu + i] = w * pw;
+            pw *= u;
+        }
+    }
+    for (int i = tid; i < nrow; i += B) {
+        const bool in = i < mc;
+        const double v = in ? P.v[m0 + i] : 0.0, w = in ? P.wv[m0 + i] : 0.0;
+        double *o = mtab + i * 6;
+        o[0] = w; o[1] = w * v; o[2] = w * v * v; o[3] = w * v * v * v; o[4] = w * v * v * v * v;
+        o[5] = v > 0.0 ? 1.0 : (v < 0.0 ? 0.0 : 0.5);
+    }
     __syncthreads();
-    if (tid == 0)
-        for (int row = rows_first; row < rows_first + NSM && row <= rows_last; ++row) issue(row);
+    if (tid == 0) {
+        for (int row = rows_first; row < rows_first + NSXM && row <= rows_last; ++row) issue_x(row);
+        issue_y(c0);
+        if (c0 + 1 < c1) issue_y(c0 + 1);
+    }
 
-    const double uk = un[k];
-    // per-thread points; points outside the chunk are clamped onto a valid one and get zero weight
-    double vreg[NPT], wreg[NPT], fm[NPT], fc[NPT];
-    int qo[NPT];
+    // per-thread points; a point outside the chunk (ragged tail, padding threads) reads a valid value and the zero weight row
+    int qoff[NPT], woff[NPT];
 #pragma unroll
     for (int p = 0; p < NPT; ++p) {
         const int mm = r + p * R;
         const bool valid = active && mm < mc;
-        qo[p] = valid ? mm * Nu + k : 0;
-        vreg[p] = vn[valid ? mm : 0];
-        wreg[p] = valid ? wvn[mm] : 0.0;
+        qoff[p] = valid ? qsh + mm * Nu + k : qsh;
+        woff[p] = (valid ? mm : nrow - 1) * 6;
     }
-    // window shift per point: 0 for n >= 0 (rows a-2, a-1 held, row a read), 1 for n < 0 (rows a-1, a held, a+1 read)
-    auto nvel = [&](int p) { return DIR == 0 ? uk : vreg[p]; };
+    double fc[NPT], dm[NPT];
     {
-        wait_row(a0 - 2); wait_row(a0 - 1); wait_row(a0);
+        wait_x(c0 - 1); wait_x(c0);
+        const double *ra = xring, *rb = xring + Qb;
 #pragma unroll
-        for (int p = 0; p < NPT; ++p) {
-            const int sh = nvel(p) < 0.0 ? 1 : 0;
-            fm[p] = ring[(size_t)sh * Qs + qo[p]];
-            fc[p] = ring[(size_t)(sh + 1) * Qs + qo[p]];
+        for (int p = 0; p < NPT; ++p) { fc[p] = rb[qoff[p]]; dm[p] = fc[p] - ra[qoff[p]]; }
+    }
+    __syncthreads();                                                 // rows c0-1, c0 consumed
+    if (tid == 0) {
+        if (c0 + 2 <= rows_last) issue_x(c0 + 2);
+        if (c0 + 3 <= rows_last) issue_x(c0 + 3);
+    }
+    const bool ym_miss = beyond_wall<1>(P, j - 1), yp_miss = beyond_wall<1>(P, j + 1);
+    const double sy = ch.z > 0 ? 1.0 : -1.0;                         // side of the y-contribution (uniform chunks)
+
+    // stage-3 descriptors: output v = (set, idx) -> (factor table, column sums ca (+- cb)); groups of nsplit lanes share an output
+    const int nsplit = B >= 4 * NOUT ? 4 : (B >= 2 * NOUT ? 2 : 1);
+    const int ngroup = B / nsplit, ov = tid / nsplit, oh = tid % nsplit;
+    const int oiter = (NOUT + ngroup - 1) / ngroup;
+    for (int v = tid; v < NOUT; v += B) {
+        int set = v / NRAW;
+        const int idx = v % NRAW;
+        int fi, ca, cb, sb;
+        if (set < 2) {                                               // x+ / x-: M terms take C_b +- B_b, S terms B_b
+            const int c = c_xc[idx];
+            fi = (set == 0 ? 0 : 5) + c_xa[idx];
+            if (c < 3) { ca = c; cb = 3 + c; sb = set == 0 ? 1 : 2; }
+            else { ca = c; cb = c; sb = 0; }
+        } else {                                                     // y (uniform chunks: one set; mixed: y+ then y-)
+            fi = 10 + c_yt[idx];
+            ca = cb = 6 + (set - 2) * 7 + c_yc[idx];
+            sb = 0;
+            if (!MIXED) set = ch.z > 0 ? 2 : 3;
         }
+        desc[v] = make_int4(fi * Nu, ca * Nu, cb * Nu, (sb << 16) | (set * NRAW + idx));
     }
     __syncthreads();
-    if (tid == 0) {
-        if (a0 + NSM - 2 <= rows_last) issue(a0 + NSM - 2);
-        if (a0 + NSM - 1 <= rows_last) issue(a0 + NSM - 1);
-    }
-    const double inv_h = 2.0 / (DIR == 0 ? P.dx : P.dy);
 
-    const int nw3 = min(nwarp, (Nu + 31) / 32);                     // warps that own columns in stage 3
-    for (int a = a0; a < a1 + 3; ++a) {
-        if (a < a1) {                                               // stage 1: point sums of face a
-            wait_row(a + 1);
-            const double *rA = ring + (size_t)((a - rows_first) % NSM) * Qs;          // row a
-            const double *rB = ring + (size_t)((a + 1 - rows_first) % NSM) * Qs;      // row a+1
-            const int ms = miss_mask_m<DIR>(P, a);
-            double acc[NACC];
+    for (int a = c0; a < c1 + 2; ++a) {
+        if (a < c1) {                                                // stage 1: point sums of cell a
+            wait_x(a + 1);
+            mbar_wait(&bars[NSXM + ((a - c0) & 1)], ((a - c0) >> 1) & 1);
+            const double *xn = xring + (size_t)((a + 1 - rows_first) % NSXM) * Qb;
+            const double *ym = ybuf + (size_t)(((a - c0) & 1) * 2) * Qb, *yp = ym + Qb;
+            const bool xm_miss = beyond_wall<0>(P, a - 1), xp_miss = beyond_wall<0>(P, a + 1);
+            double acc[NA];
 #pragma unroll
-            for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+            for (int i = 0; i < NA; ++i) acc[i] = 0.0;
             auto pass = [&](auto fl) {
                 constexpr bool FL = decltype(fl)::value;
 #pragma unroll
                 for (int p = 0; p < NPT; ++p) {
-                    const double n = nvel(p), vm = vreg[p];
-                    const bool neg = n < 0.0;
-                    const double fn = neg ? rB[qo[p]] : rA[qo[p]];
-                    double f0, hs;
-                    if (neg) recon_m<FL>(fm[p], fc[p], fn, -1.0, ms & 2, ms & 4, ms & 8, f0, hs);
-                    else recon_m<FL>(fm[p], fc[p], fn, 1.0, ms & 1, ms & 2, ms & 4, f0, hs);
-                    if (n == 0.0) {                                 // AMB-5: H(0) = 1/2, both sides; sigma0 is never used (x n)
-                        double f0r, hsr;
-                        recon_m<FL>(fc[p], fn, rB[qo[p]], -1.0, ms & 2, ms & 4, ms & 8, f0r, hsr);
-                        f0 = (FL && (ms & 6)) ? 0.0 : 0.5 * (f0 + f0r);
-                        hs = 0.0;
+                    const double fn = xn[qoff[p]], c = fc[p];
+                    const double dp = fn - c;
+                    double dxm = dm[p], dxp = dp, dym = c - ym[qoff[p]], dyp = yp[qoff[p]] - c;
+                    if (FL) {                                        // AMB-13: one-sided slope next to a wall
+                        if (xm_miss) dxm = dp; if (xp_miss) dxp = dm[p];
+                        if (ym_miss) dym = dyp; if (yp_miss) dyp = dym;
                     }
-                    fm[p] = fc[p]; fc[p] = fn;
-                    const double pw = wreg[p] * f0, sg = wreg[p] * hs, v2 = vm * vm;
-                    if (DIR == 0) {                                 // loop variable is t = v_m
-                        acc[0] += pw; acc[1] = fma(pw, vm, acc[1]); acc[2] = fma(pw, v2, acc[2]);
-                        acc[3] += sg; acc[4] = fma(sg, vm, acc[4]); acc[5] = fma(sg, v2, acc[5]);
-                    } else {                                        // loop variable is n = v_m
-                        const double pn = pw * vm, sn2 = sg * v2;
-                        acc[0] += pw; acc[1] += pn; acc[2] = fma(pn, vm, acc[2]); acc[3] = fma(pn, v2, acc[3]);
-                        acc[4] += sn2; acc[5] = fma(sn2, vm, acc[5]); acc[6] = fma(sn2, v2, acc[6]);
+                    const double hx = vl_half(dxm, dxp), hy = vl_half(dym, dyp);
+                    dm[p] = dp; fc[p] = fn;
+                    const double2 w01 = *reinterpret_cast<const double2 *>(mtab + woff[p]);
+                    const double2 w23 = *reinterpret_cast<const double2 *>(mtab + woff[p] + 2);
+                    const double2 w4h = *reinterpret_cast<const double2 *>(mtab + woff[p] + 4);
+                    // x-faces: t = v_m;  C_b = sum wv t^b f_c,  B_b = sum wv t^b h sigma
+                    acc[0] = fma(w01.x, c, acc[0]); acc[1] = fma(w01.y, c, acc[1]); acc[2] = fma(w23.x, c, acc[2]);
+                    acc[3] = fma(w01.x, hx, acc[3]); acc[4] = fma(w01.y, hx, acc[4]); acc[5] = fma(w23.x, hx, acc[5]);
+                    // y-faces: n = v_m;  A_a = sum wv n^a f0 (a = 0..3),  B_a = sum wv n^a h sigma (a = 2..4)
+                    if (!MIXED) {
+                        const double f0 = fma(sy, hy, c);
+                        acc[6] = fma(w01.x, f0, acc[6]); acc[7] = fma(w01.y, f0, acc[7]); acc[8] = fma(w23.x, f0, acc[8]);
+                        acc[9] = fma(w23.y, f0, acc[9]);
+                        acc[10] = fma(w23.x, hy, acc[10]); acc[11] = fma(w23.y, hy, acc[11]); acc[12] = fma(w4h.x, hy, acc[12]);
+                    } else {                                         // AMB-5: H(0) = 1/2 sends half of the point to either side
+                        const double hp = w4h.y, hm = 1.0 - hp, fp = (c + hy) * hp, fm = (c - hy) * hm, gp = hy * hp, gm = hy * hm;
+                        acc[6] = fma(w01.x, fp, acc[6]); acc[7] = fma(w01.y, fp, acc[7]); acc[8] = fma(w23.x, fp, acc[8]);
+                        acc[9] = fma(w23.y, fp, acc[9]);
+                        acc[10] = fma(w23.x, gp, acc[10]); acc[11] = fma(w23.y, gp, acc[11]); acc[12] = fma(w4h.x, gp, acc[12]);
+                        acc[13] = fma(w01.x, fm, acc[13]); acc[14] = fma(w01.y, fm, acc[14]); acc[15] = fma(w23.x, fm, acc[15]);
+                        acc[16] = fma(w23.y, fm, acc[16]);
+                        acc[17] = fma(w23.x, gm, acc[17]); acc[18] = fma(w23.y, gm, acc[18]); acc[19] = fma(w4h.x, gm, acc[19]);
                     }
                 }
             };
-            if (ms == 0) pass(std::false_type{}); else pass(std::true_type{});
-            double *pp = part + (size_t)(a & 1) * NACC * B + tid;
+            if (xm_miss || xp_miss || ym_miss || yp_miss) pass(std::true_type{}); else pass(std::false_type{});
+            double *pp = part + (size_t)(a & 1) * NA * B + tid;
 #pragma unroll
-            for (int i = 0; i < NACC; ++i) pp[i * B] = active ? acc[i] : 0.0;
+            for (int i = 0; i < NA; ++i) pp[i * B] = acc[i];
         }
-        if (a - 1 >= a0 && a - 1 < a1) {                            // stage 2: column sums of face a-1
-            const double *pp = part + (size_t)((a - 1) & 1) * NACC * B;
-            double *cc = col + (size_t)((a - 1) & 1) * NACC * Nu;
-            for (int idx = tid; idx < NACC * Nu; idx += B) {
+        if (a - 1 >= c0 && a - 1 < c1) {                            // stage 2: column sums of cell a-1
+            const double *pp = part + (size_t)((a - 1) & 1) * NA * B;
+            double *cc = col + (size_t)((a - 1) & 1) * NA * Nu;
+            for (int idx = tid; idx < NA * Nu; idx += B) {
                 const int i = idx / Nu, kk = idx - i * Nu;
-                double sum = 0.0;
-                for (int rr = 0; rr < R; ++rr) sum += pp[i * B + rr * Nu + kk];
+                double sum = pp[i * B + kk];
+                for (int rr = 1; rr < R; ++rr) sum += pp[i * B + rr * Nu + kk];
                 cc[idx] = sum;
             }
         }
-        if (a - 2 >= a0 && a - 2 < a1 && warp < nw3) {              // stage 3: k-dependent factors + butterfly, per warp
-            const double *cc = col + (size_t)(a & 1) * NACC * Nu;   // (a-2)&1 == a&1
-            double o[16];
-#pragma unroll
-            for (int v = 0; v < 16; ++v) o[v] = 0.0;
-            for (int kk = tid; kk < Nu; kk += 32 * nw3) {
-                const double w = wun[kk], c = un[kk], c2 = c * c, ws = w * inv_h;
-                const double A0 = cc[kk], A1 = cc[Nu + kk], A2 = cc[2 * Nu + kk], A3 = cc[3 * Nu + kk];
-                const double B4 = cc[4 * Nu + kk], B5 = cc[5 * Nu + kk], B6 = cc[6 * Nu + kk];
-                double M00, M10, M01, M20, M02, M11, M30, M12, S20, S30, S21, S40, S22;
-                if (DIR == 0) {                                     // n = u_k = c; A0..A2 = sum wv t^b f0, A3,B4,B5 = sum wv t^b hs
-                    M00 = w * A0; M10 = M00 * c; M20 = M10 * c; M30 = M20 * c;
-                    M01 = w * A1; M11 = M01 * c; M02 = w * A2; M12 = M02 * c;
-                    S20 = ws * c2 * A3; S30 = S20 * c; S40 = S30 * c; S21 = ws * c2 * B4; S22 = ws * c2 * B5;
-                } else {                                            // t = u_k = c; A0..A3 = sum wv n^a f0, B4..B6 = sum wv n^(2..4) hs
-                    M00 = w * A0; M01 = M00 * c; M02 = M01 * c;
-                    M10 = w * A1; M11 = M10 * c; M12 = M11 * c; M20 = w * A2; M30 = w * A3;
-                    S20 = ws * B4; S21 = S20 * c; S22 = S21 * c; S30 = ws * B5; S40 = ws * B6;
+        if (a - 2 >= c0) {                                           // stage 3: dot products over k of cell a-2
+            const double *cc = col + (size_t)(a & 1) * NA * Nu;      // (a-2)&1 == a&1
+            const size_t cell = (size_t)j * P.I + (a - 2);
+            double *dst = P.cmom + (cell * P.nchunk + chunk) * CMS;
+            for (int it = 0; it < oiter; ++it) {
+                const int v = it * ngroup + ov;
+                const bool on = v < NOUT;
+                const int4 d = desc[on ? v : 0];
+                const double sb = (d.w >> 16) == 0 ? 0.0 : ((d.w >> 16) == 1 ? 1.0 : -1.0);
+                double sum = 0.0;
+                if (on) {
+                    const double *F = fac + d.x, *ca = cc + d.y, *cb = cc + d.z;
+                    for (int kk = oh; kk < Nu; kk += nsplit) sum = fma(F[kk], fma(sb, cb[kk], ca[kk]), sum);
                 }
-                o[0] += M00; o[1] += M10; o[2] += M01; o[3] += 0.5 * (M20 + M02); o[4] += M20; o[5] += M11;
-                o[6] += 0.5 * (M30 + M12); o[7] += S20; o[8] += S30; o[9] += S21; o[10] += 0.5 * (S40 + S22);
+                if (nsplit >= 2) sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+                if (nsplit >= 4) sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+                if (on && oh == 0) dst[d.w & 0xffff] = sum;
             }
-            // transposing butterfly: after the step with offset 2^b the lane keeps the half selected by its bit b
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const bool hi = lane & 16;
-                const double send = hi ? o[i] : o[i + 8], keep = hi ? o[i + 8] : o[i];
-                o[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-            }
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const bool hi = lane & 8;
-                const double send = hi ? o[i] : o[i + 4], keep = hi ? o[i + 4] : o[i];
-                o[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-            }
-#pragma unroll
-            for (int i = 0; i < 2; ++i) {
-                const bool hi = lane & 4;
-                const double send = hi ? o[i] : o[i + 2], keep = hi ? o[i + 2] : o[i];
-                o[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-            }
-            {
-                const bool hi = lane & 2;
-                const double send = hi ? o[0] : o[1], keep = hi ? o[1] : o[0];
-                o[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
-            }
-            o[0] += __shfl_xor_sync(0xffffffffu, o[0], 1);
-            // lane holds moment v = 8*bit4 + 4*bit3 + 2*bit2 + bit1
-            const int v = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
-            if ((lane & 1) == 0) red[((a & 1) * 32 + warp) * 16 + v] = o[0];
-        }
-        if (a - 3 >= a0 && tid < 11) {                              // stage 4: sum over the warps of stage 3, store
-            const double *rr = red + (size_t)((a - 1) & 1) * 32 * 16 + tid;   // (a-3)&1 == (a-1)&1
-            double sum = 0.0;
-            for (int w = 0; w < nw3; ++w) sum += rr[w * 16];
-            const int fa = a - 3;
-            const size_t face = DIR == 0 ? (size_t)line * (P.I + 1) + fa : (size_t)fa * P.I + line;
-            P.mom[DIR][(face * P.nchunk + chunk) * NMOM + tid] = sum;
         }
         __syncthreads();
-        if (tid == 0 && a < a1 && a + NSM <= rows_last) issue(a + NSM);   // row a is consumed by every thread
+        if (tid == 0 && a < c1) {
+            if (a + 4 <= rows_last) issue_x(a + 4);                  // row a+1 is consumed by every thread
+            if (a + 2 < c1) issue_y(a + 2);
+        }
     }
-}
-
-size_t smem_face_moments(const UgksParams &P)
-{
-    const size_t Qs = ((size_t)P.chunk_m * P.Nu + 1) & ~(size_t)1;
-    const size_t B = ((size_t)P.Nu * P.R + 31) / 32 * 32;
-    const size_t tabs = 2 * (size_t)P.Nu + 2 * (size_t)P.chunk_m;
-    return (NSM * Qs + 2 * NACC * B + 2 * NACC * (size_t)P.Nu + tabs + 2 * 32 * 16) * sizeof(double) + NSM * sizeof(uint64_t);
 }
 
 static int block_threads(const UgksParams &P) { return ((P.Nu * P.R + 31) / 32) * 32; }
 
-template <int DIR, int MAXT, int MINB>
-static void launch_dir(const UgksParams &P, int cur, int grid, int T, size_t smem, cudaStream_t st)
+template <bool MIXED>
+static size_t smem_cm(const UgksParams &P)
+{
+    const size_t NA = MIXED ? 20 : 13, NOUT = MIXED ? 4 * NRAW : 3 * NRAW, B = block_threads(P), Qb = pad2(P.cmax * P.Nu + 1);
+    const size_t nrow = (size_t)P.R * P.npt + 1;
+    return ((NSXM + 4) * Qb + 2 * NA * B + 2 * NA * (size_t)P.Nu + pad2(NFAC * P.Nu) + pad2(nrow * 6) + 2 * NOUT) * sizeof(double)
+           + (NSXM + 2) * sizeof(uint64_t);
+}
+size_t smem_cell_moments(const UgksParams &P) { return smem_cm<true>(P); }
+
+template <bool MIXED, int MAXT, int MINB>
+static void launch_cm(const UgksParams &P, int cur, int chunk0, int grid, int T, size_t smem, cudaStream_t st)
 {
     switch (P.npt) {
-#define CASE(N) case N: k_face_moments<DIR, N, MAXT, MINB><<<grid, T, smem, st>>>(P, cur); break;
-        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#define CASE(N) case N: k_cell_moments<N, MIXED, MAXT, MINB><<<grid, T, smem, st>>>(P, cur, chunk0); break;
+        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7)
 #undef CASE
     }
 }
-
-int launch_face_moments(const UgksParams &P, int cur, int dir, cudaStream_t st)
+template <bool MIXED>
+static void launch_cm_class(const UgksParams &P, int cur, int chunk0, int nch, cudaStream_t st)
 {
-    const size_t smem = smem_face_moments(P);
-    const int nsx = (P.I + 1 + P.strip - 1) / P.strip, nsy = (P.J + 1 + P.strip - 1) / P.strip;
+    const int nstrip = (P.I + P.strip - 1) / P.strip;
     const int T = block_threads(P);
-    const int grid = dir == 0 ? P.J * nsx * P.nchunk : P.I * nsy * P.nchunk;
-    if (T <= 128) { if (dir == 0) launch_dir<0, 128, 4>(P, cur, grid, T, smem, st); else launch_dir<1, 128, 4>(P, cur, grid, T, smem, st); }
-    else if (T <= 256) { if (dir == 0) launch_dir<0, 256, 2>(P, cur, grid, T, smem, st); else launch_dir<1, 256, 2>(P, cur, grid, T, smem, st); }
-    else { if (dir == 0) launch_dir<0, 1024, 1>(P, cur, grid, T, smem, st); else launch_dir<1, 1024, 1>(P, cur, grid, T, smem, st); }
-    return 1;
+    const int grid = P.J * nstrip * nch;
+    const size_t smem = smem_cm<MIXED>(P);
+    if (T <= 64) launch_cm<MIXED, 64, 6>(P, cur, chunk0, grid, T, smem, st);
+    else if (T <= 128) launch_cm<MIXED, 128, 4>(P, cur, chunk0, grid, T, smem, st);
+    else launch_cm<MIXED, 256, 2>(P, cur, chunk0, grid, T, smem, st);
 }
 
-template <int DIR, int MAXT, int MINB>
-static cudaError_t set_attr_dir(int smem)
+int launch_cell_moments(const UgksParams &P, int cur, cudaStream_t st)
+{
+    int n = 0;
+    if (P.nneg + P.npos) { launch_cm_class<false>(P, cur, 0, P.nneg + P.npos, st); ++n; }
+    if (P.nmix) { launch_cm_class<true>(P, cur, P.nneg + P.npos, P.nmix, st); ++n; }
+    return n;
+}
+
+template <bool MIXED, int MAXT, int MINB>
+static cudaError_t set_attr_cm(int smem)
 {
     cudaError_t e = cudaSuccess;
-#define ATTR(N) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_face_moments<DIR, N, MAXT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    ATTR(1) ATTR(2) ATTR(3) ATTR(4) ATTR(5) ATTR(6) ATTR(7) ATTR(8)
+#define ATTR(N) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cell_moments<N, MIXED, MAXT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    ATTR(1) ATTR(2) ATTR(3) ATTR(4) ATTR(5) ATTR(6) ATTR(7)
 #undef ATTR
     return e;
 }
-
+template <bool MIXED>
+static cudaError_t set_attr_cm_all(int smem)
+{
+    cudaError_t e = set_attr_cm<MIXED, 64, 6>(smem);
+    if (e == cudaSuccess) e = set_attr_cm<MIXED, 128, 4>(smem);
+    if (e == cudaSuccess) e = set_attr_cm<MIXED, 256, 2>(smem);
+    return e;
+}
 int setup_moments_attributes(const UgksParams &P)
 {
-    const int smem = (int)smem_face_moments(P);
-    cudaError_t e = set_attr_dir<0, 128, 4>(smem);
-    if (e == cudaSuccess) e = set_attr_dir<1, 128, 4>(smem);
-    if (e == cudaSuccess) e = set_attr_dir<0, 256, 2>(smem);
-    if (e == cudaSuccess) e = set_attr_dir<1, 256, 2>(smem);
-    if (e == cudaSuccess) e = set_attr_dir<0, 1024, 1>(smem);
-    if (e == cudaSuccess) e = set_attr_dir<1, 1024, 1>(smem);
+    if (smem_cm<true>(P) > 227 * 1024) return 1;
+    cudaError_t e = set_attr_cm_all<false>((int)smem_cm<false>(P));
+    if (e == cudaSuccess) e = set_attr_cm_all<true>((int)smem_cm<true>(P));
     return e == cudaSuccess ? 0 : 1;
 }

@@ -87,16 +87,43 @@ __device__ void cell_W_and_tgrad(const UgksParams &P, const double *W, int pos, 
 
 __device__ __forceinline__ void swap12(double w[4]) { const double t = w[1]; w[1] = w[2]; w[2] = t; }
 
+// raw half-range sums (set `set`) of the cell at `pos` on `line`, added over the chunks that feed that set
+template <int DIR>
+__device__ __forceinline__ void add_cell_raw(const UgksParams &P, int pos, int line, int set, double raw[NRAW])
+{
+    const size_t cell = DIR == 0 ? (size_t)line * P.I + pos : (size_t)pos * P.I + line;
+    const double *cm = P.cmom + cell * P.nchunk * CMS + set * NRAW;
+    for (int c = 0; c < P.nchunk; ++c) {
+        const int sg = P.chunks[c].z;
+        if (set == 2 && sg < 0) continue;                            // a chunk of v < 0 rows holds no y+ part
+        if (set == 3 && sg > 0) continue;
+        for (int v = 0; v < NRAW; ++v) raw[v] += cm[c * CMS + v];
+    }
+}
+
 template <int DIR>
 __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
 {
     const size_t face = DIR == 0 ? (size_t)line * (P.I + 1) + pos : (size_t)pos * P.I + line;
+    const int n = DIR == 0 ? P.I : P.J, lo = DIR == 0 ? 0 : 2;
+    // O3 face sums = plus-side part of the left cell + minus-side part of the right cell (ghost rows: constants of O0)
+    double raw[NRAW];
+    for (int v = 0; v < NRAW; ++v) raw[v] = 0.0;
+    {
+        int pl = pos - 1, pr = pos;
+        if (pl < 0 && P.bc[lo] == BC_PERIODIC) pl += n;
+        if (pr >= n && P.bc[lo + 1] == BC_PERIODIC) pr -= n;
+        if (pl >= 0) add_cell_raw<DIR>(P, pl, line, DIR == 0 ? 0 : 2, raw);
+        else if (P.bc[lo] == BC_FIXED) for (int v = 0; v < NRAW; ++v) raw[v] += P.ghostmom[lo * NRAW + v];
+        if (pr < n) add_cell_raw<DIR>(P, pr, line, DIR == 0 ? 1 : 3, raw);
+        else if (P.bc[lo + 1] == BC_FIXED) for (int v = 0; v < NRAW; ++v) raw[v] += P.ghostmom[(lo + 1) * NRAW + v];
+    }
+    const double ih = 2.0 / (DIR == 0 ? P.dx : P.dy);
     double M[11];
-    for (int v = 0; v < 11; ++v) M[v] = 0.0;
-    const double *mp = P.mom[DIR] + face * P.nchunk * NMOM;
-    for (int c = 0; c < P.nchunk; ++c)
-        for (int v = 0; v < 11; ++v) M[v] += mp[c * NMOM + v];
-    double *cf = P.coef[DIR] + face * NCOEF, *fw = P.fw[DIR] + face * 4;
+    M[0] = raw[RW_M00]; M[1] = raw[RW_M10]; M[2] = raw[RW_M01]; M[3] = 0.5 * (raw[RW_M20] + raw[RW_M02]);
+    M[4] = raw[RW_M20]; M[5] = raw[RW_M11]; M[6] = 0.5 * (raw[RW_M30] + raw[RW_M12]);
+    M[7] = ih * raw[RW_S20]; M[8] = ih * raw[RW_S30]; M[9] = ih * raw[RW_S21]; M[10] = ih * 0.5 * (raw[RW_S40] + raw[RW_S22]);
+    double *cf = P.frec[DIR] + face * P.frs, *fw = P.fw[DIR] + face * 4;
     const double h = 0.5 * (DIR == 0 ? P.dx : P.dy), ell = DIR == 0 ? P.dy : P.dx, dt = P.dt;
 
     double WL[4], WR[4], gL[4], gR[4];
@@ -114,9 +141,9 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
         for (int r = 1; r < 4; ++r) F[r] = ell * dt * (S[r] + rho_w * G[r]);
         if (DIR == 1) swap12(F);
         for (int r = 0; r < 4; ++r) fw[r] = F[r];
-        for (int r = 0; r < NCOEF; ++r) cf[r] = 0.0;
-        cf[CF_MT4] = dt;                                             // F_q = ell n dt f_w through the common formula
-        cf[CF_TYPE] = 1.0; cf[CF_RHOW] = rho_w;
+        for (int r = 0; r < FR_NCOEF; ++r) cf[r] = 0.0;
+        cf[FR_MT4] = ell * dt;                                       // F_q = ell n dt f_w through the common formula
+        cf[FR_TYPE] = 1.0; cf[FR_RHOW] = rho_w; cf[FR_LAM] = 1.0;
         return;
     }
     if (DIR == 1) { swap12(WL); swap12(WR); swap12(gL); swap12(gR); }
@@ -186,23 +213,25 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
     if (DIR == 1) swap12(F);
     for (int r = 0; r < 4; ++r) fw[r] = F[r];
 
-    cf[CF_C0] = p0.rho * p0.lam / UGKS_PI; cf[CF_U] = p0.U; cf[CF_V] = p0.V; cf[CF_LAM] = p0.lam;
-    cf[CF_MT4] = Mt4; cf[CF_MT5] = Mt5; cf[CF_RHOW] = 0.0; cf[CF_TYPE] = 0.0;
-    cf[CF_C00] = Mt1 + Mt3 * A[0];
-    cf[CF_C01] = Mt2 * bb[0] + Mt3 * A[2];
-    cf[CF_C02] = Mt2 * bb[2] + 0.5 * Mt3 * A[3];
-    cf[CF_C03] = 0.5 * Mt2 * bb[3];
-    cf[CF_C21] = 0.5 * Mt2 * bb[3];
+    // flux polynomial ell C0 [Mt1 + Mt2 (n a.psi + t b.psi) + Mt3 A.psi] = sum c_ab n^a t^b, C0 = rho lam / pi
+    const double sc = ell * p0.rho * p0.lam / UGKS_PI;
+    cf[FR_LAM] = p0.lam; cf[FR_U] = p0.U; cf[FR_V] = p0.V; cf[FR_TYPE] = 0.0; cf[FR_RHOW] = 0.0;
+    cf[FR_MT4] = ell * Mt4; cf[FR_MT5] = -ell * Mt5 * (1.0 / h); cf[FR_TAU] = tau;
+    cf[FR_C00] = sc * (Mt1 + Mt3 * A[0]);
+    cf[FR_C01] = sc * (Mt2 * bb[0] + Mt3 * A[2]);
+    cf[FR_C02] = sc * (Mt2 * bb[2] + 0.5 * Mt3 * A[3]);
+    cf[FR_C03] = sc * (0.5 * Mt2 * bb[3]);
+    cf[FR_C21] = sc * (0.5 * Mt2 * bb[3]);
     for (int sd = 0; sd < 2; ++sd) {
         const double *a = sd == 0 ? aL : aR;
-        double *o = cf + (sd == 0 ? CF_L : CF_R);
-        o[0] = Mt2 * a[0] + Mt3 * A[1];              // c10
-        o[1] = Mt2 * a[1] + 0.5 * Mt3 * A[3];        // c20
-        o[2] = 0.5 * Mt2 * a[3];                     // c30
-        o[3] = Mt2 * (a[2] + bb[1]);                 // c11
-        o[4] = 0.5 * Mt2 * a[3];                     // c12
+        double *o = cf + (sd == 0 ? FR_L : FR_R);
+        o[LR_C10] = sc * (Mt2 * a[0] + Mt3 * A[1]);
+        o[LR_C20] = sc * (Mt2 * a[1] + 0.5 * Mt3 * A[3]);
+        o[LR_C30] = sc * (0.5 * Mt2 * a[3]);
+        o[LR_C11] = sc * (Mt2 * (a[2] + bb[1]));
+        o[LR_C12] = sc * (0.5 * Mt2 * a[3]);
     }
-    cf[23] = tau;
+    cf[23] = 0.0;
 }
 
 __global__ void __launch_bounds__(128) k_face_scalars(const UgksParams P, const int cur)
@@ -237,11 +266,12 @@ __global__ void __launch_bounds__(128) k_cell_scalars(const UgksParams P, const 
         if (!(pp.rho > 0.0) || !(pp.lam > 0.0)) atomicOr(P.status, 2);
         const double tn = tau_of(P, pn.rho, pn.lam), tp = tau_of(P, pp.rho, pp.lam);
         const double inv = 1.0 / (1.0 + 0.5 * P.dt / tp);
-        double *cc = P.cellc + (size_t)c * NCELL;
-        cc[CC_GN] = pn.rho * pn.lam / UGKS_PI * (0.5 * P.dt / tn) * inv; cc[CC_UN] = pn.U; cc[CC_VN] = pn.V; cc[CC_LN] = pn.lam;
-        cc[CC_GP] = pp.rho * pp.lam / UGKS_PI * (0.5 * P.dt / tp) * inv; cc[CC_UP] = pp.U; cc[CC_VP] = pp.V; cc[CC_LP] = pp.lam;
-        cc[CC_KF] = (1.0 - 0.5 * P.dt / tn) * inv;
-        cc[CC_KD] = iOm * inv;
+        double *cc = P.crec + (size_t)c * P.crs;
+        cc[CR_GN] = pn.rho * pn.lam / UGKS_PI * (0.5 * P.dt / tn) * inv; cc[CR_UN] = pn.U; cc[CR_VN] = pn.V; cc[CR_LN] = pn.lam;
+        cc[CR_GP] = pp.rho * pp.lam / UGKS_PI * (0.5 * P.dt / tp) * inv; cc[CR_UP] = pp.U; cc[CR_VP] = pp.V; cc[CR_LP] = pp.lam;
+        cc[CR_KF] = (1.0 - 0.5 * P.dt / tn) * inv;
+        cc[CR_KD] = iOm * inv;
+        cc[10] = 0.0; cc[11] = 0.0;
     }
     __shared__ double sh[4][8];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -280,7 +310,7 @@ __global__ void __launch_bounds__(256) k_residual_final(const double *part, int 
 
 // O0: ghost rows, wall Maxwellians, W_b and the outgoing wall sums G (one block per side)
 __global__ void __launch_bounds__(256) k_setup(const UgksParams P, const double *bcprim, double *ghost, double *wallg,
-                                               double *Wb, double *wallG)
+                                               double *Wb, double *wallG, double *ghostmom)
 {
     const int side = blockIdx.x, type = P.bc[side];
     const double rho = type == BC_FIXED ? bcprim[side * 4 + 0] : 1.0, U = bcprim[side * 4 + 1], V = bcprim[side * 4 + 2];
@@ -288,32 +318,40 @@ __global__ void __launch_bounds__(256) k_setup(const UgksParams P, const double 
     const int dir = side >> 1;
     const double sgn = (side & 1) ? 1.0 : -1.0;                      // outward normal = sgn * e_dir
     double g[4] = { 0, 0, 0, 0 };
+    double gm[8] = { 0, 0, 0, 0, 0, 0, 0, 0 };                      // raw M sums of the ghost row toward the domain (sigma = 0)
     for (int q = threadIdx.x; q < P.Npad; q += blockDim.x) {
         double val = 0.0;
         if (q < P.N && type != BC_PERIODIC) {
             const int k = q % P.Nu, m = q / P.Nu;
             const double u = P.u[k], v = P.v[m], du = u - U, dv = v - V;
             val = rho * (lam / UGKS_PI) * exp(-lam * (du * du + dv * dv));
+            const double n = dir == 0 ? u : v, t = dir == 0 ? v : u, w = P.wu[k] * P.wv[m];
             if (type == BC_WALL) {
-                const double n = dir == 0 ? u : v, t = dir == 0 ? v : u, w = P.wu[k] * P.wv[m];
                 if (sgn * n < 0.0) {                                 // leaves the wall (1-H)
                     const double wn = w * n * val;
                     g[0] += wn; g[1] += wn * n; g[2] += wn * t; g[3] += wn * 0.5 * (n * n + t * t);
                 }
+            } else if (type == BC_FIXED) {                           // part of the ghost row that enters the domain, H(0) = 1/2
+                const double hin = sgn * n < 0.0 ? 1.0 : (n == 0.0 ? 0.5 : 0.0), wf = w * hin * val;
+                gm[RW_M00] += wf; gm[RW_M10] += wf * n; gm[RW_M20] += wf * n * n; gm[RW_M30] += wf * n * n * n;
+                gm[RW_M01] += wf * t; gm[RW_M11] += wf * n * t; gm[RW_M02] += wf * t * t; gm[RW_M12] += wf * n * t * t;
             }
         }
         ghost[(size_t)side * P.Npad + q] = type == BC_FIXED ? val : 0.0;
         wallg[(size_t)side * P.Npad + q] = type == BC_WALL ? val : 0.0;
     }
-    __shared__ double sh[8][4];
+    __shared__ double sh[8][12];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int r = 0; r < 4; ++r) { const double s = warp_sum(g[r]); if (lane == 0) sh[warp][r] = s; }
+    for (int r = 0; r < 8; ++r) { const double s = warp_sum(gm[r]); if (lane == 0) sh[warp][4 + r] = s; }
     __syncthreads();
-    if (threadIdx.x < 4) {
+    if (threadIdx.x < 12) {
         double s = 0.0;
         for (int w = 0; w < 8; ++w) s += sh[w][threadIdx.x];
-        wallG[side * 4 + threadIdx.x] = s;
+        if (threadIdx.x < 4) wallG[side * 4 + threadIdx.x] = s;
+        else ghostmom[side * NRAW + threadIdx.x - 4] = s;
     }
+    if (threadIdx.x >= 8 && threadIdx.x < NRAW) ghostmom[side * NRAW + threadIdx.x] = 0.0;      // S sums: ghost rows have sigma = 0
     if (threadIdx.x == 0) {
         Wb[side * 4 + 0] = rho; Wb[side * 4 + 1] = rho * U; Wb[side * 4 + 2] = rho * V;
         Wb[side * 4 + 3] = 0.5 * rho * (U * U + V * V) + rho / (2.0 * lam);
@@ -353,9 +391,57 @@ int launch_residual_final(const UgksParams &P, int resblocks, double *res_dev, c
     return 1;
 }
 int launch_setup(const UgksParams &P, const double *bc_prims, double *ghost, double *wallg, double *Wb, double *wallG,
-                 cudaStream_t st)
+                 double *ghostmom, cudaStream_t st)
 {
-    k_setup<<<4, 256, 0, st>>>(P, bc_prims, ghost, wallg, Wb, wallG);
+    k_setup<<<4, 256, 0, st>>>(P, bc_prims, ghost, wallg, Wb, wallG, ghostmom);
+    return 1;
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_tables: every exponential of the step (S6 and the two cell equilibria of U2), once per face / cell and node:
+// exp(-lam ((u-U)^2 + (v-V)^2)) = E_k[k] E_m[m] on the tensor-product grid, so a face needs Nu + Nv exponentials, not Nu Nv.
+// One thread per table entry; the records are read back by k_flux_update through TMA.
+__global__ void __launch_bounds__(256) k_tables(const UgksParams P)
+{
+    const int nt = P.NuP + P.NvP;                                    // entries per Maxwellian
+    const long nfx = nfaces_x(P), nfy = nfaces_y(P), ncell = (long)P.I * P.J;
+    const long total = (nfx + nfy + 2 * ncell) * nt;
+    for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
+        const long rec = g / nt;
+        const int e = (int)(g - rec * nt);
+        const bool isk = e < P.NuP;
+        const int idx = isk ? e : e - P.NuP;
+        const bool pad = isk ? idx >= P.Nu : idx >= P.Nv;
+        const double node = pad ? 0.0 : (isk ? P.u[idx] : P.v[idx]);
+        double lam, cen, pref = 1.0, *dst;
+        bool zero = pad;
+        if (rec < nfx + nfy) {                                       // face Maxwellian (local frame: U normal, V tangential)
+            const int dir = rec >= nfx;
+            double *fr = P.frec[dir] + (dir ? rec - nfx : rec) * P.frs;
+            lam = fr[FR_LAM];
+            cen = (isk == (dir == 0)) ? fr[FR_U] : fr[FR_V];         // x-face: u is normal; y-face: v is normal
+            zero = zero || fr[FR_TYPE] != 0.0;                       // wall faces carry no equilibrium part
+            dst = fr + FR_NCOEF + e;
+        } else {                                                     // cell equilibria g^n (w = 0), g^{n+1} (w = 1)
+            const long cw = rec - nfx - nfy, cell = cw >> 1;
+            const int w = (int)(cw & 1);
+            double *cr = P.crec + cell * P.crs;
+            lam = cr[w ? CR_LP : CR_LN];
+            cen = isk ? cr[w ? CR_UP : CR_UN] : cr[w ? CR_VP : CR_VN];
+            if (isk) pref = cr[w ? CR_GP : CR_GN];
+            dst = cr + CR_NCOEF + (isk ? w * P.NuP + idx : 2 * P.NuP + w * P.NvP + idx);
+        }
+        const double d = node - cen;
+        *dst = zero ? 0.0 : pref * exp(-lam * d * d);
+    }
+}
+
+int launch_tables(const UgksParams &P, cudaStream_t st)
+{
+    const long total = ((long)nfaces_x(P) + nfaces_y(P) + 2L * P.I * P.J) * (P.NuP + P.NvP);
+    long blocks = (total + 255) / 256;
+    if (blocks > 148L * 64) blocks = 148L * 64;
+    k_tables<<<(int)blocks, 256, 0, st>>>(P);
     return 1;
 }
 int launch_moments_of_f(const UgksParams &P, const double *f, double *Wf, cudaStream_t st)

@@ -17,7 +17,7 @@ struct ugks_ctx {
     double *res_dev, *bcprim_dev, *Wf_dev;
     double *ghost, *wallg, *Wb, *wallG, *ghostmom;   // non-const aliases of the P fields
     int4 *chunks_dev;
-    double *vhost;            // host copy of the v nodes (chunking)
+    double *vhost, *uhost;    // host copies of the velocity nodes (chunking, column ranges by sign)
     size_t cells;
     int profile;              // option "profile": time every kernel of ugks_step with CUDA events
     cudaEvent_t *ev; int nev, nev_used;
@@ -155,6 +155,19 @@ static int apply_geometry(ugks_ctx *c, const Chunking *C, int R, int npt, int nc
     UgksParams T = c->P;
     T.nchunk = C->n; T.nneg = C->nneg; T.npos = C->npos; T.nmix = C->nmix; T.cmax = C->cmax; T.R = R; T.npt = npt;
     if (C->n > nchunk_alloc) return fail(c, UGKS_EINVAL, "%s", "too many chunks for the allocated moment buffer");
+    {   // columns by sign of u (sorted nodes), and the stage-3 split of k_cell_moments
+        bool sorted = true;
+        for (int k = 1; k < T.Nu; ++k) if (c->uhost[k] < c->uhost[k - 1]) sorted = false;
+        T.kxm_end = T.Nu; T.kxp_begin = 0;
+        if (sorted) {
+            int k0 = 0, k1 = 0;
+            while (k0 < T.Nu && c->uhost[k0] < 0.0) ++k0;            // first u >= 0
+            k1 = k0; while (k1 < T.Nu && c->uhost[k1] <= 0.0) ++k1;  // first u > 0
+            T.kxp_begin = k0; T.kxm_end = k1;
+        }
+        const int lenx = T.kxm_end > T.Nu - T.kxp_begin ? T.kxm_end : T.Nu - T.kxp_begin;
+        choose_stage3_split(T.Nu, lenx, (T.Nu * R + 31) / 32 * 32, C->nmix > 0, &T.s3_nsx, &T.s3_nsy);
+    }
     if (npt < 1 || npt > 7 || R < 1 || T.Nu * R > 256 || R * npt < C->cmax) return fail(c, UGKS_EINVAL, "%s", "R / points per thread out of range");
     if (smem_flux_update(T) > 227 * 1024 || smem_cell_moments(T) > 227 * 1024) return fail(c, UGKS_EINVAL, "%s", "chunk does not fit in shared memory");
     for (int i = 0; i < C->n; ++i)
@@ -242,6 +255,9 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     c->vhost = (double *)malloc(sizeof(double) * vg->Nv);
     if (!c->vhost) { free(c); return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed"); }
     memcpy(c->vhost, vg->v, sizeof(double) * vg->Nv);
+    c->uhost = (double *)malloc(sizeof(double) * vg->Nu);
+    if (!c->uhost) { free(c->vhost); free(c); return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed"); }
+    memcpy(c->uhost, vg->u, sizeof(double) * vg->Nu);
     c->cells = (size_t)m->I * m->J;
     c->st = (cudaStream_t)cuda_stream;
     static Chunking C;
@@ -264,9 +280,9 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     if (e == cudaSuccess) e = cudaMemsetAsync(P.crec, 0, c->cells * (size_t)P.crs * 8, c->st);
     if (e == cudaSuccess) { c->launches += launch_setup(P, c->bcprim_dev, c->ghost, c->wallg, c->Wb, c->wallG, c->ghostmom, c->st); e = cudaGetLastError(); }
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
-    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); free(c->vhost); free(c); return rc; }
+    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); free(c->vhost); free(c->uhost); free(c); return rc; }
     { const int rc = apply_geometry(c, &C, R0, npt0, c->nchunk_alloc);
-      if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); free(c->vhost); free(c); return rc; } }
+      if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); free(c->vhost); free(c->uhost); free(c); return rc; } }
     *out = c;
     return UGKS_OK;
 }
@@ -278,6 +294,7 @@ void ugks_destroy(ugks_ctx *c)
     for (int i = 0; i < c->nev; ++i) cudaEventDestroy(c->ev[i]);
     free(c->ev);
     free(c->vhost);
+    free(c->uhost);
     free(c);
 }
 

@@ -63,7 +63,9 @@ struct UgksParams {
     int nneg, npos, nmix;            // chunks per class
     int cmax;                        // rows of the largest chunk
     int R;                           // velocity rows processed in parallel by one CTA (threads = Nu*R rounded up to 32)
-    int npt;                         // velocity points per thread = ceil(cmax / R), 1..8 (template parameter)
+    int npt;                         // velocity points per thread = ceil(cmax / R), 1..7 (template parameter)
+    int kxm_end, kxp_begin;          // columns with u_k <= 0 are [0, kxm_end), with u_k >= 0 [kxp_begin, Nu) (sorted nodes; else 0..Nu)
+    int s3_nsx, s3_nsy;              // k_cell_moments stage 3: parts per x-output / y-output dot product
 };
 
 static __host__ __device__ inline int nfaces_x(const UgksParams &P) { return (P.I + 1) * P.J; }
@@ -91,6 +93,25 @@ __device__ __forceinline__ const double *row_ptr(const UgksParams &P, const doub
     const size_t cell = DIR == 0 ? (size_t)line * P.I + pos : (size_t)pos * P.I + line;
     return f + cell * P.Npad;
 }
+// y-neighbour row `pos` of column 0 and its stride (doubles) from cell to cell along x: Npad, or 0 for a ghost row
+__device__ __forceinline__ const double *yrow_base(const UgksParams &P, const double *f, int pos, int *stride)
+{
+    *stride = P.Npad;
+    if (pos < 0) {
+        if (P.bc[2] == BC_PERIODIC) pos += P.J;
+        else if (P.bc[2] == BC_FIXED) { *stride = 0; return P.ghost + (size_t)2 * P.Npad; }
+        else pos = 0;
+    } else if (pos >= P.J) {
+        if (P.bc[3] == BC_PERIODIC) pos -= P.J;
+        else if (P.bc[3] == BC_FIXED) { *stride = 0; return P.ghost + (size_t)3 * P.Npad; }
+        else pos = P.J - 1;
+    }
+    return f + (size_t)pos * P.I * P.Npad;
+}
+// shared-memory load at a byte offset from a (warp-uniform) base: LDS R, [Roff + URbase]
+__device__ __forceinline__ double ldsd(const unsigned char *base, int off) { return *reinterpret_cast<const double *>(base + off); }
+__device__ __forceinline__ double2 ldsd2(const unsigned char *base, int off) { return *reinterpret_cast<const double2 *>(base + off); }
+
 // is cell `pos` of a line beyond a WALL side?
 template <int DIR>
 __device__ __forceinline__ bool beyond_wall(const UgksParams &P, int pos)
@@ -161,4 +182,5 @@ int launch_moments_of_f(const UgksParams &P, const double *f, double *Wf, cudaSt
 int setup_moments_attributes(const UgksParams &P);
 int setup_update_attributes(const UgksParams &P);
 size_t smem_cell_moments(const UgksParams &P);
+void choose_stage3_split(int Nu, int lenx, int B, bool any_mixed, int *nsx, int *nsy);
 size_t smem_flux_update(const UgksParams &P);

@@ -10,24 +10,51 @@
 // allows, so that the y-side of a point is CTA-uniform).  Thread (k, r) owns velocity column k and the rows m = r + p*R.
 //   * x-stencil: (f_c, f_c - f_{c-1}) live in registers; ONE new row per cell comes from a 3-slot shared-memory ring fed by
 //     1-D TMA bulk copies (cp.async.bulk + mbarrier).  y-neighbours (i, j-1), (i, j+1): TMA-staged, double-buffered.
-//   * sums are tensor products: a thread accumulates sum_m wv v^p (.) for its column (13 sums; weights wv v^p come as
-//     broadcast shared-memory loads); three pipelined stages, one per cell step, finish the reduction without an extra
-//     barrier: (1) partial sums to shared memory, (2) sum over the R threads of a column, (3) per output one thread (or
-//     2 / 4) takes the dot product over k with the factors wu u^a H(+-u).
+//   * sums are tensor products: a thread accumulates sum_m wv v^p (.) for its column (13 sums; the weights wv v^p come as
+//     broadcast shared-memory loads).  Four pipelined stages, one per cell step and one barrier per step, finish the
+//     reduction: (1) partial sums to shared memory; (2) sum over the R threads of a column, forming C_b +- B_b for the two
+//     x-sides; (3) balanced work items (output, k-range): dot product over k with the factors wu u^a H(+-u);
+//     (4) one thread per output adds its items and stores.
 #include "ugks_common.cuh"
 #include <type_traits>
 
 constexpr int NSXM = 3;                                              // x-ring slots
 constexpr int NFAC = 13;                                             // factor tables: 5 (x+), 5 (x-), 3 (y)
-__constant__ int c_xa[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 2, 3, 4, 2, 2 };   // power of n = u_k of raw sum idx (x sets)
-__constant__ int c_xc[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 3, 3, 3, 4, 5 };   // column sum: 0..2 = C_b (+- B_b), 3..5 = B_b
-__constant__ int c_yt[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 0, 0, 0, 1, 2 };   // power of t = u_k (y sets)
-__constant__ int c_yc[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 4, 5, 6, 4, 4 };   // column sum: A_0..A_3, B_2..B_4
+// raw sum idx -> (power of the per-column velocity, column sum) ; x sets: columns 0..2 = C_b +- B_b, 3..5 = B_b
+__constant__ int c_xa[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 2, 3, 4, 2, 2 };
+__constant__ int c_xc[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 3, 3, 3, 4, 5 };
+__constant__ int c_yt[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 0, 0, 0, 1, 2 };   // y sets: columns A_0..A_3, B_2..B_4
+__constant__ int c_yc[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 4, 5, 6, 4, 4 };
+
+struct MomLayout {                                                   // shared-memory carve-up (offsets in doubles)
+    int ybuf, part, col, fac, mtab, ires, desc, odesc, bars, NuS, nitem, bytes;
+};
+__host__ __device__ inline MomLayout mom_layout(bool mixed, int Nu, int cmax, int R, int npt, int B, int nsx, int nsy)
+{
+    const int NA = mixed ? 20 : 13, NC = mixed ? 23 : 16, NOUT = mixed ? 4 * NRAW : 3 * NRAW;
+    const int Qb = pad2(cmax * Nu + 1), nrow = R * npt + 1;
+    MomLayout L;
+    L.NuS = Nu | 1;                                                  // odd column stride: conflict-free across columns
+    L.nitem = 2 * NRAW * nsx + (mixed ? 2 : 1) * NRAW * nsy;
+    int o = NSXM * Qb;
+    L.ybuf = o; o += 4 * Qb;
+    L.part = o; o += 2 * NA * B;
+    L.col = o; o += pad2(2 * NC * L.NuS);
+    L.fac = o; o += pad2(NFAC * L.NuS);
+    L.mtab = o; o += pad2(nrow * 6);
+    L.ires = o; o += pad2(2 * L.nitem);
+    L.desc = o; o += 2 * L.nitem;                                    // int4 per item
+    L.odesc = o; o += 2 * NOUT;                                      // int4 per output
+    L.bars = o; o += NSXM + 2;
+    L.bytes = o * 8;
+    return L;
+}
 
 template <int NPT, bool MIXED, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P, const int cur, const int chunk0)
 {
-    constexpr int NA = MIXED ? 20 : 13;                              // column sums per thread: 6 (x) + 7 (y) [+ 7 (y-)]
+    constexpr int NA = MIXED ? 20 : 13;                              // per-thread sums: 6 (x) + 7 (y) [+ 7 (y-)]
+    constexpr int NC = MIXED ? 23 : 16;                              // columns after stage 2: 9 (x) + 7 (y) [+ 7]
     constexpr int NOUT = MIXED ? 4 * NRAW : 3 * NRAW;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int nstrip = (P.I + P.strip - 1) / P.strip;
@@ -40,31 +67,37 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
     const int m0 = ch.x, mc = ch.y;
     const int Nu = P.Nu, R = P.R;
     const int q0 = m0 * Nu, qa = q0 & ~1, qsh = q0 - qa;             // 16-byte aligned copy start; shift of the chunk inside
-    const int Qb = pad2(P.cmax * Nu + 1);
+    const int Qb = pad2(P.cmax * Nu + 1), QbB = Qb * 8;
     const uint32_t bytes = (uint32_t)(pad2(mc * Nu + qsh) * sizeof(double));
     const int B = blockDim.x;
     const int nrow = R * NPT + 1;                                    // weight rows incl. a zero row
+    const MomLayout L = mom_layout(MIXED, Nu, P.cmax, R, NPT, B, P.s3_nsx, P.s3_nsy);
+    const int NuS = L.NuS, nitem = L.nitem;
 
-    double *xring = reinterpret_cast<double *>(smem_raw);            // [NSXM][Qb]
-    double *ybuf = xring + (size_t)NSXM * Qb;                        // [2][2][Qb]
-    double *part = ybuf + (size_t)4 * Qb;                            // [2][NA][B]
-    double *col = part + (size_t)2 * NA * B;                         // [2][NA][Nu]
-    double *fac = col + (size_t)2 * NA * Nu;                         // [NFAC][Nu]
-    double *mtab = fac + (size_t)pad2(NFAC * Nu);                    // [nrow][6]: w, w v, w v^2, w v^3, w v^4, H(v)
-    int4 *desc = reinterpret_cast<int4 *>(mtab + (size_t)pad2(nrow * 6));      // [NOUT] stage-3 output descriptors
-    uint64_t *bars = reinterpret_cast<uint64_t *>(desc + NOUT);     // [NSXM] x rows, [2] y stages
+    double *sm = reinterpret_cast<double *>(smem_raw);
+    double *xring = sm;                                              // [NSXM][Qb]
+    double *ybuf = sm + L.ybuf;                                      // [2][2][Qb]
+    double *part = sm + L.part;                                      // [2][NA][B]
+    double *col = sm + L.col;                                        // [2][NC][NuS]
+    double *fac = sm + L.fac;                                        // [NFAC][NuS]
+    double *mtab = sm + L.mtab;                                      // [nrow][6]: w, w v, w v^2, w v^3, w v^4, H(v)
+    double *ires = sm + L.ires;                                      // [2][nitem] stage-3 item results
+    int4 *desc = reinterpret_cast<int4 *>(sm + L.desc);              // [nitem]  (fac offset, col offset, k begin, k end)
+    int4 *odesc = reinterpret_cast<int4 *>(sm + L.odesc);            // [NOUT]   (first item, items, set*NRAW+idx, 0)
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sm + L.bars);      // [NSXM] x rows, [2] y stages
 
     const int tid = threadIdx.x;
     const bool active = tid < Nu * R;
     const int k = active ? tid % Nu : 0, r = active ? tid / Nu : 0;
     const double *fcur = P.f[cur];
     const int rows_first = c0 - 1, rows_last = c1;                   // cells c0-1 .. c1 are staged
+    int ystm, ystp;
+    const double *ybm = yrow_base(P, fcur, j - 1, &ystm) + qa, *ybp = yrow_base(P, fcur, j + 1, &ystp) + qa;
 
     auto issue_x = [&](int row) {
         const int sl = (row - rows_first) % NSXM;
-        const double *src = row_ptr<0>(P, fcur, row, j) + qa;
         mbar_expect_tx(&bars[sl], bytes);
-        tma_load_1d(xring + (size_t)sl * Qb, src, bytes, &bars[sl]);
+        tma_load_1d(xring + (size_t)sl * Qb, row_ptr<0>(P, fcur, row, j) + qa, bytes, &bars[sl]);
     };
     auto wait_x = [&](int row) {
         const int idx = row - rows_first;
@@ -73,8 +106,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
     auto issue_y = [&](int cell) {
         const int buf = (cell - c0) & 1;
         mbar_expect_tx(&bars[NSXM + buf], 2 * bytes);
-        tma_load_1d(ybuf + (size_t)(buf * 2) * Qb, row_ptr<1>(P, fcur, j - 1, cell) + qa, bytes, &bars[NSXM + buf]);
-        tma_load_1d(ybuf + (size_t)(buf * 2 + 1) * Qb, row_ptr<1>(P, fcur, j + 1, cell) + qa, bytes, &bars[NSXM + buf]);
+        tma_load_1d(ybuf + (size_t)(buf * 2) * Qb, ybm + (size_t)cell * ystm, bytes, &bars[NSXM + buf]);
+        tma_load_1d(ybuf + (size_t)(buf * 2 + 1) * Qb, ybp + (size_t)cell * ystp, bytes, &bars[NSXM + buf]);
     };
 
     if (tid == 0) {
@@ -86,9 +119,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
         const double hp = u > 0.0 ? 1.0 : (u < 0.0 ? 0.0 : 0.5);
         double pw = 1.0;
         for (int a = 0; a < 5; ++a) {
-            fac[a * Nu + i] = w * hp * pw;
-            fac[(5 + a) * Nu + i] = w * (1.0 - hp) * pw;
-            if (a < 3) fac[(10 + a) * Nu + i] = w * pw;
+            fac[a * NuS + i] = w * hp * pw;
+            fac[(5 + a) * NuS + i] = w * (1.0 - hp) * pw;
+            if (a < 3) fac[(10 + a) * NuS + i] = w * pw;
             pw *= u;
         }
     }
@@ -99,6 +132,29 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
         o[0] = w; o[1] = w * v; o[2] = w * v * v; o[3] = w * v * v * v; o[4] = w * v * v * v * v;
         o[5] = v > 0.0 ? 1.0 : (v < 0.0 ? 0.0 : 0.5);
     }
+    // stage-3 work items: output v = (set, idx) split into ns parts of its k-range; x+ sums u_k >= 0, x- sums u_k <= 0
+    for (int v = tid; v < NOUT; v += B) {
+        int set = v / NRAW;
+        const int idx = v % NRAW;
+        int fi, ci, kb, ke, ns, first;
+        if (set < 2) {
+            const int c = c_xc[idx];
+            fi = (set == 0 ? 0 : 5) + c_xa[idx];
+            ci = c < 3 ? (set == 0 ? c : 3 + c) : 3 + c;             // columns: 0..2 C+B, 3..5 C-B, 6..8 B
+            kb = set == 0 ? P.kxp_begin : 0; ke = set == 0 ? Nu : P.kxm_end;
+            ns = P.s3_nsx; first = v * ns;
+        } else {
+            fi = 10 + c_yt[idx];
+            ci = 9 + (set - 2) * 7 + c_yc[idx];
+            kb = 0; ke = Nu;
+            ns = P.s3_nsy; first = 2 * NRAW * P.s3_nsx + (v - 2 * NRAW) * ns;
+            if (!MIXED) set = ch.z > 0 ? 2 : 3;
+        }
+        const int len = ke - kb, per = (len + ns - 1) / ns;
+        for (int h = 0; h < ns; ++h)
+            desc[first + h] = make_int4(fi * NuS * 8, ci * NuS * 8, min(kb + h * per, ke), min(kb + (h + 1) * per, ke));
+        odesc[v] = make_int4(first, ns, set * NRAW + idx, 0);
+    }
     __syncthreads();
     if (tid == 0) {
         for (int row = rows_first; row < rows_first + NSXM && row <= rows_last; ++row) issue_x(row);
@@ -106,21 +162,24 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
         if (c0 + 1 < c1) issue_y(c0 + 1);
     }
 
-    // per-thread points; a point outside the chunk (ragged tail, padding threads) reads a valid value and the zero weight row
-    int qoff[NPT], woff[NPT];
+    // per-thread points (byte offsets); a point outside the chunk (ragged tail, padding threads) reads a valid value and
+    // the zero weight row
+    int qb[NPT], wb[NPT];
 #pragma unroll
     for (int p = 0; p < NPT; ++p) {
         const int mm = r + p * R;
         const bool valid = active && mm < mc;
-        qoff[p] = valid ? qsh + mm * Nu + k : qsh;
-        woff[p] = (valid ? mm : nrow - 1) * 6;
+        qb[p] = (valid ? qsh + mm * Nu + k : qsh) * 8;
+        wb[p] = (valid ? mm : nrow - 1) * 48;
     }
+    const unsigned char *xring_b = reinterpret_cast<const unsigned char *>(xring);
+    const unsigned char *ybuf_b = reinterpret_cast<const unsigned char *>(ybuf);
+    const unsigned char *mtab_b = reinterpret_cast<const unsigned char *>(mtab);
     double fc[NPT], dm[NPT];
     {
         wait_x(c0 - 1); wait_x(c0);
-        const double *ra = xring, *rb = xring + Qb;
 #pragma unroll
-        for (int p = 0; p < NPT; ++p) { fc[p] = rb[qoff[p]]; dm[p] = fc[p] - ra[qoff[p]]; }
+        for (int p = 0; p < NPT; ++p) { fc[p] = ldsd(xring_b + QbB, qb[p]); dm[p] = fc[p] - ldsd(xring_b, qb[p]); }
     }
     __syncthreads();                                                 // rows c0-1, c0 consumed
     if (tid == 0) {
@@ -129,36 +188,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
     }
     const bool ym_miss = beyond_wall<1>(P, j - 1), yp_miss = beyond_wall<1>(P, j + 1);
     const double sy = ch.z > 0 ? 1.0 : -1.0;                         // side of the y-contribution (uniform chunks)
+    constexpr int NJ = NC - 6;                                       // stage-2 jobs per column: 3 (x, b = 0..2) + 7 (y) [+ 7]
 
-    // stage-3 descriptors: output v = (set, idx) -> (factor table, column sums ca (+- cb)); groups of nsplit lanes share an output
-    const int nsplit = B >= 4 * NOUT ? 4 : (B >= 2 * NOUT ? 2 : 1);
-    const int ngroup = B / nsplit, ov = tid / nsplit, oh = tid % nsplit;
-    const int oiter = (NOUT + ngroup - 1) / ngroup;
-    for (int v = tid; v < NOUT; v += B) {
-        int set = v / NRAW;
-        const int idx = v % NRAW;
-        int fi, ca, cb, sb;
-        if (set < 2) {                                               // x+ / x-: M terms take C_b +- B_b, S terms B_b
-            const int c = c_xc[idx];
-            fi = (set == 0 ? 0 : 5) + c_xa[idx];
-            if (c < 3) { ca = c; cb = 3 + c; sb = set == 0 ? 1 : 2; }
-            else { ca = c; cb = c; sb = 0; }
-        } else {                                                     // y (uniform chunks: one set; mixed: y+ then y-)
-            fi = 10 + c_yt[idx];
-            ca = cb = 6 + (set - 2) * 7 + c_yc[idx];
-            sb = 0;
-            if (!MIXED) set = ch.z > 0 ? 2 : 3;
-        }
-        desc[v] = make_int4(fi * Nu, ca * Nu, cb * Nu, (sb << 16) | (set * NRAW + idx));
-    }
-    __syncthreads();
-
-    for (int a = c0; a < c1 + 2; ++a) {
+    for (int a = c0; a < c1 + 3; ++a) {
         if (a < c1) {                                                // stage 1: point sums of cell a
             wait_x(a + 1);
             mbar_wait(&bars[NSXM + ((a - c0) & 1)], ((a - c0) >> 1) & 1);
-            const double *xn = xring + (size_t)((a + 1 - rows_first) % NSXM) * Qb;
-            const double *ym = ybuf + (size_t)(((a - c0) & 1) * 2) * Qb, *yp = ym + Qb;
+            const unsigned char *xn = xring_b + ((a + 1 - rows_first) % NSXM) * QbB;
+            const unsigned char *ym = ybuf_b + ((a - c0) & 1) * 2 * QbB, *yp = ym + QbB;
             const bool xm_miss = beyond_wall<0>(P, a - 1), xp_miss = beyond_wall<0>(P, a + 1);
             double acc[NA];
 #pragma unroll
@@ -167,18 +204,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
                 constexpr bool FL = decltype(fl)::value;
 #pragma unroll
                 for (int p = 0; p < NPT; ++p) {
-                    const double fn = xn[qoff[p]], c = fc[p];
+                    const double fn = ldsd(xn, qb[p]), c = fc[p];
                     const double dp = fn - c;
-                    double dxm = dm[p], dxp = dp, dym = c - ym[qoff[p]], dyp = yp[qoff[p]] - c;
+                    double dxm = dm[p], dxp = dp, dym = c - ldsd(ym, qb[p]), dyp = ldsd(yp, qb[p]) - c;
                     if (FL) {                                        // AMB-13: one-sided slope next to a wall
                         if (xm_miss) dxm = dp; if (xp_miss) dxp = dm[p];
                         if (ym_miss) dym = dyp; if (yp_miss) dyp = dym;
                     }
                     const double hx = vl_half(dxm, dxp), hy = vl_half(dym, dyp);
                     dm[p] = dp; fc[p] = fn;
-                    const double2 w01 = *reinterpret_cast<const double2 *>(mtab + woff[p]);
-                    const double2 w23 = *reinterpret_cast<const double2 *>(mtab + woff[p] + 2);
-                    const double2 w4h = *reinterpret_cast<const double2 *>(mtab + woff[p] + 4);
+                    const double2 w01 = ldsd2(mtab_b, wb[p]), w23 = ldsd2(mtab_b + 16, wb[p]), w4h = ldsd2(mtab_b + 32, wb[p]);
                     // x-faces: t = v_m;  C_b = sum wv t^b f_c,  B_b = sum wv t^b h sigma
                     acc[0] = fma(w01.x, c, acc[0]); acc[1] = fma(w01.y, c, acc[1]); acc[2] = fma(w23.x, c, acc[2]);
                     acc[3] = fma(w01.x, hx, acc[3]); acc[4] = fma(w01.y, hx, acc[4]); acc[5] = fma(w23.x, hx, acc[5]);
@@ -204,33 +239,39 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
 #pragma unroll
             for (int i = 0; i < NA; ++i) pp[i * B] = acc[i];
         }
-        if (a - 1 >= c0 && a - 1 < c1) {                            // stage 2: column sums of cell a-1
-            const double *pp = part + (size_t)((a - 1) & 1) * NA * B;
-            double *cc = col + (size_t)((a - 1) & 1) * NA * Nu;
-            for (int idx = tid; idx < NA * Nu; idx += B) {
-                const int i = idx / Nu, kk = idx - i * Nu;
-                double sum = pp[i * B + kk];
-                for (int rr = 1; rr < R; ++rr) sum += pp[i * B + rr * Nu + kk];
-                cc[idx] = sum;
+        if (a - 1 >= c0 && a - 1 < c1 && active) {                  // stage 2: column sums of cell a-1
+            const double *pp = part + (size_t)((a - 1) & 1) * NA * B + k;
+            double *cc = col + (size_t)((a - 1) & 1) * NC * NuS + k;
+            for (int jb = r; jb < NJ; jb += R) {
+                if (jb < 3) {                                        // x, power b = jb of t: C_b +- B_b for the two sides, B_b
+                    double C = pp[jb * B], Bs = pp[(3 + jb) * B];
+                    for (int rr = 1; rr < R; ++rr) { C += pp[jb * B + rr * Nu]; Bs += pp[(3 + jb) * B + rr * Nu]; }
+                    cc[jb * NuS] = C + Bs; cc[(3 + jb) * NuS] = C - Bs; cc[(6 + jb) * NuS] = Bs;
+                } else {                                             // y sums
+                    double A = pp[(3 + jb) * B];
+                    for (int rr = 1; rr < R; ++rr) A += pp[(3 + jb) * B + rr * Nu];
+                    cc[(6 + jb) * NuS] = A;
+                }
             }
         }
-        if (a - 2 >= c0) {                                           // stage 3: dot products over k of cell a-2
-            const double *cc = col + (size_t)(a & 1) * NA * Nu;      // (a-2)&1 == a&1
-            const size_t cell = (size_t)j * P.I + (a - 2);
-            double *dst = P.cmom + (cell * P.nchunk + chunk) * CMS;
-            for (int it = 0; it < oiter; ++it) {
-                const int v = it * ngroup + ov;
-                const bool on = v < NOUT;
-                const int4 d = desc[on ? v : 0];
-                const double sb = (d.w >> 16) == 0 ? 0.0 : ((d.w >> 16) == 1 ? 1.0 : -1.0);
+        if (a - 2 >= c0 && a - 2 < c1) {                            // stage 3: items (output, k-range) of cell a-2
+            const unsigned char *cc = reinterpret_cast<const unsigned char *>(col + (size_t)(a & 1) * NC * NuS);   // (a-2)&1 == a&1
+            const unsigned char *fb = reinterpret_cast<const unsigned char *>(fac);
+            for (int it = tid; it < nitem; it += B) {
+                const int4 d = desc[it];
                 double sum = 0.0;
-                if (on) {
-                    const double *F = fac + d.x, *ca = cc + d.y, *cb = cc + d.z;
-                    for (int kk = oh; kk < Nu; kk += nsplit) sum = fma(F[kk], fma(sb, cb[kk], ca[kk]), sum);
-                }
-                if (nsplit >= 2) sum += __shfl_xor_sync(0xffffffffu, sum, 1);
-                if (nsplit >= 4) sum += __shfl_xor_sync(0xffffffffu, sum, 2);
-                if (on && oh == 0) dst[d.w & 0xffff] = sum;
+                for (int kk = d.z; kk < d.w; ++kk) sum = fma(ldsd(fb + d.x, kk * 8), ldsd(cc + d.y, kk * 8), sum);
+                ires[(a & 1) * nitem + it] = sum;
+            }
+        }
+        if (a - 3 >= c0) {                                           // stage 4: add the items of each output of cell a-3, store
+            const double *ir = ires + ((a - 1) & 1) * nitem;         // (a-3)&1 == (a-1)&1
+            double *dst = P.cmom + (((size_t)j * P.I + (a - 3)) * P.nchunk + chunk) * CMS;
+            for (int v = tid; v < NOUT; v += B) {
+                const int4 od = odesc[v];
+                double sum = ir[od.x];
+                for (int h = 1; h < od.y; ++h) sum += ir[od.x + h];
+                dst[od.z] = sum;
             }
         }
         __syncthreads();
@@ -246,12 +287,22 @@ static int block_threads(const UgksParams &P) { return ((P.Nu * P.R + 31) / 32) 
 template <bool MIXED>
 static size_t smem_cm(const UgksParams &P)
 {
-    const size_t NA = MIXED ? 20 : 13, NOUT = MIXED ? 4 * NRAW : 3 * NRAW, B = block_threads(P), Qb = pad2(P.cmax * P.Nu + 1);
-    const size_t nrow = (size_t)P.R * P.npt + 1;
-    return ((NSXM + 4) * Qb + 2 * NA * B + 2 * NA * (size_t)P.Nu + pad2(NFAC * P.Nu) + pad2(nrow * 6) + 2 * NOUT) * sizeof(double)
-           + (NSXM + 2) * sizeof(uint64_t);
+    return (size_t)mom_layout(MIXED, P.Nu, P.cmax, P.R, P.npt, block_threads(P), P.s3_nsx, P.s3_nsy).bytes;
 }
 size_t smem_cell_moments(const UgksParams &P) { return smem_cm<true>(P); }
+
+// stage-3 split: the fewest parts per output (nsx for the 26 x-outputs over ~Nu/2 columns, nsy for the y-outputs over Nu
+// columns) such that items have about equal length and fit one pass of the CTA's threads
+void choose_stage3_split(int Nu, int lenx, int B, bool any_mixed, int *nsx, int *nsy)
+{
+    const int ny = any_mixed ? 2 * NRAW : NRAW;
+    int best_x = 1, best_y = 1;
+    for (int per = 1; per <= Nu; ++per) {                            // columns per item
+        const int sx = (lenx + per - 1) / per, sy = (Nu + per - 1) / per;
+        if (2 * NRAW * sx + ny * sy <= B) { best_x = sx; best_y = sy; break; }
+    }
+    *nsx = best_x; *nsy = best_y;
+}
 
 template <bool MIXED, int MAXT, int MINB>
 static void launch_cm(const UgksParams &P, int cur, int chunk0, int grid, int T, size_t smem, cudaStream_t st)

@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
     const int q0 = m0 * Nu, qa = q0 & ~1, qsh = q0 - qa;             // 16-byte aligned copy start; shift of the chunk inside
     const int Qb = pad2(P.cmax * Nu + 1), QbB = Qb * 8;
     const uint32_t bytes = (uint32_t)(pad2(mc * Nu + qsh) * sizeof(double));
-    const int B = blockDim.x;
+    const int B = blockDim.x - 32;                                   // compute threads; the last warp is the TMA producer
     const int nrow = R * NPT + 1;                                    // weight rows incl. a zero row
     const MomLayout L = mom_layout(MIXED, Nu, P.cmax, R, NPT, B, P.s3_nsx, P.s3_nsy);
     const int NuS = L.NuS, nitem = L.nitem;
@@ -114,6 +114,28 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
         for (int i = 0; i < NSXM + 2; ++i) mbar_init(&bars[i], 1);
         mbar_fence_init();
     }
+    if (tid >= B) {                                                  // ---- producer warp: one lane issues every bulk copy
+        const bool lead = tid == B;
+        __syncthreads();                                             // barriers initialised, tables written
+        if (lead) {
+            for (int row = rows_first; row < rows_first + NSXM && row <= rows_last; ++row) issue_x(row);
+            issue_y(c0);
+            if (c0 + 1 < c1) issue_y(c0 + 1);
+        }
+        __syncthreads();                                             // rows c0-1, c0 consumed
+        if (lead) {
+            if (c0 + 2 <= rows_last) issue_x(c0 + 2);
+            if (c0 + 3 <= rows_last) issue_x(c0 + 3);
+        }
+        for (int a = c0; a < c1 + 3; ++a) {
+            __syncthreads();                                         // step a done: row a+1 and y stage a are free
+            if (lead && a < c1) {
+                if (a + 4 <= rows_last) issue_x(a + 4);
+                if (a + 2 < c1) issue_y(a + 2);
+            }
+        }
+        return;
+    }
     for (int i = tid; i < Nu; i += B) {
         const double u = P.u[i], w = P.wu[i];
         const double hp = u > 0.0 ? 1.0 : (u < 0.0 ? 0.0 : 0.5);
@@ -156,11 +178,6 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
         odesc[v] = make_int4(first, ns, set * NRAW + idx, 0);
     }
     __syncthreads();
-    if (tid == 0) {
-        for (int row = rows_first; row < rows_first + NSXM && row <= rows_last; ++row) issue_x(row);
-        issue_y(c0);
-        if (c0 + 1 < c1) issue_y(c0 + 1);
-    }
 
     // per-thread points (byte offsets); a point outside the chunk (ragged tail, padding threads) reads a valid value and
     // the zero weight row
@@ -182,10 +199,6 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
         for (int p = 0; p < NPT; ++p) { fc[p] = ldsd(xring_b + QbB, qb[p]); dm[p] = fc[p] - ldsd(xring_b, qb[p]); }
     }
     __syncthreads();                                                 // rows c0-1, c0 consumed
-    if (tid == 0) {
-        if (c0 + 2 <= rows_last) issue_x(c0 + 2);
-        if (c0 + 3 <= rows_last) issue_x(c0 + 3);
-    }
     const bool ym_miss = beyond_wall<1>(P, j - 1), yp_miss = beyond_wall<1>(P, j + 1);
     const double sy = ch.z > 0 ? 1.0 : -1.0;                         // side of the y-contribution (uniform chunks)
     constexpr int NJ = NC - 6;                                       // stage-2 jobs per column: 3 (x, b = 0..2) + 7 (y) [+ 7]
@@ -259,8 +272,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
             const unsigned char *fb = reinterpret_cast<const unsigned char *>(fac);
             for (int it = tid; it < nitem; it += B) {
                 const int4 d = desc[it];
+                const double *pf = reinterpret_cast<const double *>(fb + d.x) + d.z, *pc = reinterpret_cast<const double *>(cc + d.y) + d.z;
                 double sum = 0.0;
-                for (int kk = d.z; kk < d.w; ++kk) sum = fma(ldsd(fb + d.x, kk * 8), ldsd(cc + d.y, kk * 8), sum);
+#pragma unroll 4
+                for (int n = d.w - d.z; n > 0; --n) sum = fma(*pf++, *pc++, sum);
                 ires[(a & 1) * nitem + it] = sum;
             }
         }
@@ -274,11 +289,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
                 dst[od.z] = sum;
             }
         }
-        __syncthreads();
-        if (tid == 0 && a < c1) {
-            if (a + 4 <= rows_last) issue_x(a + 4);                  // row a+1 is consumed by every thread
-            if (a + 2 < c1) issue_y(a + 2);
-        }
+        __syncthreads();                                             // row a+1 is consumed by every thread
     }
 }
 
@@ -317,12 +328,12 @@ template <bool MIXED>
 static void launch_cm_class(const UgksParams &P, int cur, int chunk0, int nch, cudaStream_t st)
 {
     const int nstrip = (P.I + P.strip - 1) / P.strip;
-    const int T = block_threads(P);
+    const int T = block_threads(P) + 32;                             // + producer warp
     const int grid = P.J * nstrip * nch;
     const size_t smem = smem_cm<MIXED>(P);
-    if (T <= 64) launch_cm<MIXED, 64, 6>(P, cur, chunk0, grid, T, smem, st);
-    else if (T <= 128) launch_cm<MIXED, 128, 4>(P, cur, chunk0, grid, T, smem, st);
-    else launch_cm<MIXED, 256, 2>(P, cur, chunk0, grid, T, smem, st);
+    if (T <= 96) launch_cm<MIXED, 96, 4>(P, cur, chunk0, grid, T, smem, st);
+    else if (T <= 160) launch_cm<MIXED, 160, 3>(P, cur, chunk0, grid, T, smem, st);
+    else launch_cm<MIXED, 288, 1>(P, cur, chunk0, grid, T, smem, st);
 }
 
 int launch_cell_moments(const UgksParams &P, int cur, cudaStream_t st)
@@ -345,9 +356,9 @@ static cudaError_t set_attr_cm(int smem)
 template <bool MIXED>
 static cudaError_t set_attr_cm_all(int smem)
 {
-    cudaError_t e = set_attr_cm<MIXED, 64, 6>(smem);
-    if (e == cudaSuccess) e = set_attr_cm<MIXED, 128, 4>(smem);
-    if (e == cudaSuccess) e = set_attr_cm<MIXED, 256, 2>(smem);
+    cudaError_t e = set_attr_cm<MIXED, 96, 4>(smem);
+    if (e == cudaSuccess) e = set_attr_cm<MIXED, 160, 3>(smem);
+    if (e == cudaSuccess) e = set_attr_cm<MIXED, 288, 1>(smem);
     return e;
 }
 int setup_moments_attributes(const UgksParams &P)

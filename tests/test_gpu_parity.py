@@ -141,3 +141,36 @@ def test_device_pointers_and_errors():
     g.step(1)
     with pytest.raises(UgksError):
         g.sync()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C5", "C4"])
+def test_full_size_sampled_cells_one_step(name):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (default geometry): one GPU step, then
+    sampled cells (corners, wall rows, inflow/outflow columns, strip seams, interior) against the oracle's one-by-one
+    ``cell_update`` from the same initial state; plus properties that hold at any size (finite, W of the boundary rows)."""
+    import psutil
+    from oracle import Oracle
+    from paper_1810_08137_b200 import Ugks
+    p = workloads.channel_config(name)
+    need = p.points * 8 * 3.3
+    if psutil.virtual_memory().available < need:
+        pytest.skip(f"host RAM too small for the oracle state of {name} ({need / 1e9:.0f} GB)")
+    W, f, _ = workloads.initial_state(p)
+    g = Ugks(p)
+    g.set_state(W, f)
+    g.step(1)
+    Wg = g.W()
+    fg = g.f()
+    assert np.isfinite(Wg).all() and np.isfinite(fg).all()
+    o = Oracle(p, threads=8)
+    o.set_state(W, f)
+    rng = np.random.default_rng(7)
+    cells = {(0, 0), (p.I - 1, 0), (0, p.J - 1), (p.I - 1, p.J - 1), (1, 1), (p.I - 2, p.J - 2), (31, 3), (32, 3), (33, p.J // 2)}
+    cells |= {(int(rng.integers(p.I)), int(rng.integers(p.J))) for _ in range(12)}
+    ef = eW = 0.0
+    for (i, j) in sorted(cells):
+        Wn, fn = o.cell_update(i, j)
+        fn = np.asarray(fn).reshape(p.Nv, p.Nu)
+        ef = max(ef, float(np.max(np.abs(fg[j, i] - fn)) / np.max(np.abs(fn))))
+        eW = max(eW, err_W(Wg[j, i][None], np.asarray(Wn)[None]))
+    assert ef <= TOL_1 and eW <= TOL_1, (ef, eW)

@@ -29,6 +29,7 @@ import workloads  # noqa: E402
 METRIC = "fp64 UGKS cell x velocity-point updates/s"
 UNIT = "updates/s"
 ALG_BYTES_PER_POINT = 16.0          # read f^n once, write f^{n+1} once
+FP64_PEAK = 148 * 4 * 16 * 1.965e9  # plain FP64 pipe, thread-instructions/s (one warp DFMA per 2 cycles per sub-partition)
 
 
 def _peaks():
@@ -251,9 +252,15 @@ def main():
     dom = max(r["kernels"], key=lambda k: r["kernels"][k]["ms_per_launch"])
     share = {k: v["ms_per_launch"] for k, v in r["kernels"].items()}
     tot = sum(share.values())
-    # bytes the dominant kernel must move per launch: flux_update reads f once and writes f once (16 B/pt);
-    # a face_moments launch reads f once (8 B/pt).  DESIGN.md "Roofline".
+    # bytes the dominant kernel must move per step: flux_update reads f once and writes f once (16 B/pt);
+    # cell_moments reads f once (8 B/pt).  DESIGN.md "Roofline".
     dom_bytes = (16.0 if dom == "flux_update" else 8.0) * p.points
+    traffic = None                                              # dram bytes of that kernel per step from the committed ncu capture
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            traffic = json.load(fh).get(p.name, {}).get(dom)
+    except Exception:
+        pass
     achieved = dom_bytes / (r["kernels"][dom]["ms_per_launch"] * 1e-3) / 1e9
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": r["ms"] / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -263,7 +270,9 @@ def main():
                        if p.points * 8 > 126e6 else "L2-resident workload (f = %.0f MB), no flush" % (p.points * 8 / 1e6)},
             "clocks": r["clocks"], "gpu_launches": r["launches"],
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                         "fp64": {"peak_thread_inst_per_s": FP64_PEAK, "note": "148 SMs x 4 x 16 lanes x 1.965 GHz (DESIGN.md 5)",
+                                  "step_frac_at_100_inst_per_update": value / world * 100.0 / FP64_PEAK},
                          "kernel_share_of_step": share[dom] / tot,
                          "kernel_ms": {k: round(v, 5) for k, v in share.items()},
                          "step_frac_of_16B_floor": ALG_BYTES_PER_POINT * value / world / 1e9 / peak},

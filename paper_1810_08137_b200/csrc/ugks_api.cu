@@ -99,6 +99,7 @@ static void choose_R(int Nu, int cmax, int *R, int *npt)
 static void choose_geometry(const double *v, int I, int J, int Nu, int Nv, Chunking *C, int *R, int *npt, int *strip)
 {
     int cm = 800 / Nu; if (cm < 1) cm = 1; if (cm > 56) cm = 56;
+    if (Nu > 128 && cm < 7) cm = 7;                                  // wide rows: one thread per column, 7 points per thread
     make_chunks(v, Nv, Nu, cm, C);
     choose_R(Nu, C->cmax, R, npt);
     int s = 32;

@@ -38,7 +38,7 @@ __host__ __device__ inline MomLayout mom_layout(bool mixed, int Nu, int cmax, in
     L.nitem = 2 * NRAW * nsx + (mixed ? 2 : 1) * NRAW * nsy;
     int o = NSXM * Qb;
     L.ybuf = o; o += 4 * Qb;
-    L.part = o; o += 2 * NA * B;
+    L.part = o; o += R == 1 ? 0 : 2 * NA * B;                        // R = 1: a thread owns its column, stage 1 writes the columns
     L.col = o; o += pad2(2 * NC * L.NuS);
     L.fac = o; o += pad2(NFAC * L.NuS);
     L.mtab = o; o += pad2(nrow * 6);
@@ -201,6 +201,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
     __syncthreads();                                                 // rows c0-1, c0 consumed
     const bool ym_miss = beyond_wall<1>(P, j - 1), yp_miss = beyond_wall<1>(P, j + 1);
     const double sy = ch.z > 0 ? 1.0 : -1.0;                         // side of the y-contribution (uniform chunks)
+    const int s3lag = R == 1 ? 1 : 2;                                // pipeline lag of stage 3 behind stage 1
     constexpr int NJ = NC - 6;                                       // stage-2 jobs per column: 3 (x, b = 0..2) + 7 (y) [+ 7]
 
     for (int a = c0; a < c1 + 3; ++a) {
@@ -248,11 +249,23 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
                 }
             };
             if (xm_miss || xp_miss || ym_miss || yp_miss) pass(std::true_type{}); else pass(std::false_type{});
-            double *pp = part + (size_t)(a & 1) * NA * B + tid;
+            if (R == 1) {                                            // the thread's sums are the column sums: stage 2 folded in
+                if (active) {
+                    double *cc = col + (size_t)(a & 1) * NC * NuS + k;
 #pragma unroll
-            for (int i = 0; i < NA; ++i) pp[i * B] = acc[i];
+                    for (int bb = 0; bb < 3; ++bb) {
+                        cc[bb * NuS] = acc[bb] + acc[3 + bb]; cc[(3 + bb) * NuS] = acc[bb] - acc[3 + bb]; cc[(6 + bb) * NuS] = acc[3 + bb];
+                    }
+#pragma unroll
+                    for (int i = 6; i < NA; ++i) cc[(3 + i) * NuS] = acc[i];
+                }
+            } else {
+                double *pp = part + (size_t)(a & 1) * NA * B + tid;
+#pragma unroll
+                for (int i = 0; i < NA; ++i) pp[i * B] = acc[i];
+            }
         }
-        if (a - 1 >= c0 && a - 1 < c1 && active) {                  // stage 2: column sums of cell a-1
+        if (R > 1 && a - 1 >= c0 && a - 1 < c1 && active) {         // stage 2: column sums of cell a-1
             const double *pp = part + (size_t)((a - 1) & 1) * NA * B + k;
             double *cc = col + (size_t)((a - 1) & 1) * NC * NuS + k;
             for (int jb = r; jb < NJ; jb += R) {
@@ -267,8 +280,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
                 }
             }
         }
-        if (a - 2 >= c0 && a - 2 < c1) {                            // stage 3: items (output, k-range) of cell a-2
-            const unsigned char *cc = reinterpret_cast<const unsigned char *>(col + (size_t)(a & 1) * NC * NuS);   // (a-2)&1 == a&1
+        const int c3 = a - s3lag, c4 = c3 - 1;
+        if (c3 >= c0 && c3 < c1) {                                   // stage 3: items (output, k-range) of cell c3
+            const unsigned char *cc = reinterpret_cast<const unsigned char *>(col + (size_t)(c3 & 1) * NC * NuS);
             const unsigned char *fb = reinterpret_cast<const unsigned char *>(fac);
             for (int it = tid; it < nitem; it += B) {
                 const int4 d = desc[it];
@@ -276,12 +290,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
                 double sum = 0.0;
 #pragma unroll 4
                 for (int n = d.w - d.z; n > 0; --n) sum = fma(*pf++, *pc++, sum);
-                ires[(a & 1) * nitem + it] = sum;
+                ires[(c3 & 1) * nitem + it] = sum;
             }
         }
-        if (a - 3 >= c0) {                                           // stage 4: add the items of each output of cell a-3, store
-            const double *ir = ires + ((a - 1) & 1) * nitem;         // (a-3)&1 == (a-1)&1
-            double *dst = P.cmom + (((size_t)j * P.I + (a - 3)) * P.nchunk + chunk) * CMS;
+        if (c4 >= c0 && c4 < c1) {                                   // stage 4: add the items of each output of cell c4, store
+            const double *ir = ires + (c4 & 1) * nitem;
+            double *dst = P.cmom + (((size_t)j * P.I + c4) * P.nchunk + chunk) * CMS;
             for (int v = tid; v < NOUT; v += B) {
                 const int4 od = odesc[v];
                 double sum = ir[od.x];

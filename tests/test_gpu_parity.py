@@ -174,3 +174,29 @@ def test_full_size_sampled_cells_one_step(name):
         ef = max(ef, float(np.max(np.abs(fg[j, i] - fn)) / np.max(np.abs(fn))))
         eW = max(eW, err_W(Wg[j, i][None], np.asarray(Wn)[None]))
     assert ef <= TOL_1 and eW <= TOL_1, (ef, eW)
+
+
+@pytest.mark.parametrize("I,J,nu,nv", [(2, 2, 4, 4), (2, 3, 6, 2), (3, 2, 2, 6), (5, 4, 1, 8), (4, 5, 8, 1), (33, 2, 12, 10)])
+def test_minimal_meshes_and_degenerate_velocity_grids(I, J, nu, nv):
+    """Smallest meshes the API accepts (every cell touches two boundaries) and one-node velocity directions,
+    periodic and with walls / fixed sides."""
+    p = workloads.periodic_box(I, J, max(nu, 2), max(nv, 2), a=4.0, Kn=0.2, seed=11)
+    if nu == 1:
+        p.u, p.wu = np.array([0.3]), np.array([1.0])
+    if nv == 1:
+        p.v, p.wv = np.array([-0.2]), np.array([1.0])
+    _check(_run_pair(p, 2), 2 * TOL_1)
+    q = workloads.channel_config("C1", I=I, J=J, Nuv=6)
+    _check(_run_pair(q, 2), 2 * TOL_1)
+
+
+def test_unsorted_and_asymmetric_velocity_nodes():
+    """Node sets that are not ascending (all chunks take the per-point path) and grids that are not symmetric about 0."""
+    p = workloads.periodic_box(7, 5, 12, 10, a=5.0, Kn=0.1, seed=12)
+    rng = np.random.default_rng(1)
+    pu, pv = rng.permutation(12), rng.permutation(10)
+    p.u, p.wu, p.v, p.wv = p.u[pu], p.wu[pu], p.v[pv], p.wv[pv]
+    _check(_run_pair(p, 3), 3 * TOL_1)
+    q = workloads.channel_config("C1", I=9, J=6, Nuv=10)
+    q.u = q.u + 0.7; q.v = q.v - 1.3                        # 7 of 10 nodes positive in u, 3 of 10 in v; W of f no longer matches: fine
+    _check(_run_pair(q, 3), 3 * TOL_1)

@@ -406,6 +406,7 @@ __global__ void __launch_bounds__(256) k_tables(const UgksParams P)
     const int nt = P.NuP + P.NvP;                                    // entries per Maxwellian
     const long nfx = nfaces_x(P), nfy = nfaces_y(P), ncell = (long)P.I * P.J;
     const long total = (nfx + nfy + 2 * ncell) * nt;
+#pragma unroll 4
     for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
         const long rec = g / nt;
         const int e = (int)(g - rec * nt);

@@ -313,7 +313,7 @@ static void launch_class(const UgksParams &P, int cur, int chunk0, int nch, cuda
     const int grid = P.J * nstrip * nch;
     const size_t smem = smem_fu(P, SGN == 0 ? 4 : 3);
     if (threads <= 96) launch_sgn<SGN, 96, 4>(P, cur, chunk0, grid, threads, smem, st);
-    else if (threads <= 160) launch_sgn<SGN, 160, 2>(P, cur, chunk0, grid, threads, smem, st);
+    else if (threads <= 160) launch_sgn<SGN, 160, 3>(P, cur, chunk0, grid, threads, smem, st);
     else launch_sgn<SGN, 288, 1>(P, cur, chunk0, grid, threads, smem, st);
 }
 
@@ -340,7 +340,7 @@ template <int SGN>
 static cudaError_t set_attr_sgn(int smem)
 {
     cudaError_t e = set_attr_all<SGN, 96, 4>(smem);
-    if (e == cudaSuccess) e = set_attr_all<SGN, 160, 2>(smem);
+    if (e == cudaSuccess) e = set_attr_all<SGN, 160, 3>(smem);
     if (e == cudaSuccess) e = set_attr_all<SGN, 288, 1>(smem);
     return e;
 }

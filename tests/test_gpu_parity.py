@@ -37,7 +37,7 @@ def _check(r, tol):
     assert err_W(r["Wf_g"], r["Wf_o"]) <= tol
 
 
-@pytest.mark.parametrize("steps,tol", [(1, TOL_1), (10, TOL_100)])
+@pytest.mark.parametrize("steps,tol", [(1, TOL_1), (10, TOL_100), (100, TOL_100)])
 def test_C1_channel(steps, tol):
     _check(_run_pair(workloads.channel_config("C1"), steps), tol)
 

@@ -97,6 +97,9 @@ int ugks_set_option(ugks_ctx *, const char *name, int value);
  * the last call, in launch order: cell_moments, face_scalars, cell_scalars, tables, flux_update.
  * Synchronises the stream and resets the accumulators. */
 int ugks_kernel_times(ugks_ctx *, double ms[5], long counts[5]);
+/* Measured throughput of the plain FP64 pipe: thread-level DFMA per second of a register-resident 8-chain kernel on the
+ * current device (the arithmetic roof quoted by bench.py beside the HBM roofline).  Takes ~10 ms. */
+int ugks_fp64_peak(double *thread_dfma_per_s);
 const char *ugks_last_error(const ugks_ctx *);           /* library-owned string; ctx may be NULL */
 const char *ugks_version(void);
 void ugks_destroy(ugks_ctx *);

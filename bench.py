@@ -299,6 +299,12 @@ def main():
                             "workload": _workload_name(q),
                             "kernel_ms": {k: round(v["ms_per_launch"], 5) for k, v in rr["kernels"].items()},
                             "step_frac_of_16B_floor": ALG_BYTES_PER_POINT * q.points * st / (rr["ms"] * 1e-3) / 1e9 / peak}
+        for mname, nuv, st in (("M4", 29, 50), ("M4", 69, 20), ("M3", 49, 30)):          # the paper's own shapes (Table 1 / Table 3)
+            q = workloads.paper_mesh(mname, nuv)
+            rr = measure(q, st, 3, e2e=False, kernels=True)
+            others[q.name] = {"value": q.points * st / (rr["ms"] * 1e-3), "ms_per_step": rr["ms"] / st, "steps": st,
+                              "workload": f"paper mesh {mname} {q.I}x{q.J}, {nuv}x{nuv} velocity grid, Kn=0.1",
+                              "kernel_ms": {k: round(v["ms_per_launch"], 5) for k, v in rr["kernels"].items()}}
         line["other_workloads"] = others
     if rank == 0:
         print(json.dumps(line), flush=True)

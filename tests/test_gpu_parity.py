@@ -207,3 +207,9 @@ def test_unsorted_and_asymmetric_velocity_nodes():
     q = workloads.channel_config("C1", I=9, J=6, Nuv=10)
     q.u = q.u + 0.7; q.v = q.v - 1.3                        # 7 of 10 nodes positive in u, 3 of 10 in v; W of f no longer matches: fine
     _check(_run_pair(q, 3), 3 * TOL_1)
+
+
+@pytest.mark.parametrize("name,nuv,steps", [("M1", 29, 5), ("M2", 49, 1), ("M1", 69, 1)])
+def test_paper_meshes_odd_grids_full_field(name, nuv, steps):
+    """The paper's own shapes (Table 1): whole-field parity on odd velocity grids with a node at 0."""
+    _check(_run_pair(workloads.paper_mesh(name, nuv), steps), max(1, steps) * TOL_1)

@@ -6,4 +6,4 @@ method's arithmetic (no reconstruction, moments, fluxes or updates).  The one fo
 is the Maxwellian used to *draw* an initial f from seeded primitive fields, Eq. (1).
 """
 from .channel import (BC_FIXED, BC_PERIODIC, BC_WALL, CONFIGS, Problem, channel_config,  # noqa: F401
-                      initial_state, maxwellian_field, periodic_box, trapezoid_grid, smooth_noise)
+                      initial_state, maxwellian_field, paper_mesh, periodic_box, trapezoid_grid, smooth_noise)

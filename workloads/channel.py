@@ -96,6 +96,22 @@ def channel_config(name: str, I: int | None = None, J: int | None = None, Nuv: i
                    name=name, seed=181008137 + int(name[1]), eps=eps, rho_drop=0.1)
 
 
+_PAPER_MESHES = {"M1": (40, 20), "M2": (80, 40), "M3": (120, 60), "M4": (160, 80)}     # P:L110-117 Table 1
+
+
+def paper_mesh(name: str, nuv: int = 29) -> Problem:
+    """The paper's own shapes: mesh M1..M4 of Table 1 with an odd nuv x nuv velocity grid (29, 49, 69:
+    P:L115-117, L140; a node at u = 0 and at v = 0), Kn = 0.1, same channel recipe as C1..C5.  The paper does not
+    state its velocity range or quadrature rule (AMB-16): [-5, 5]^2, [-6, 6]^2, [-7, 7]^2 with trapezoid weights here."""
+    I, J = _PAPER_MESHES[name]
+    a = {29: 5.0, 49: 6.0, 69: 7.0}.get(nuv, 5.0)
+    u, wu = trapezoid_grid(nuv, a)
+    v, wv = trapezoid_grid(nuv, a)
+    return Problem(I=I, J=J, x0=0.0, x1=2.0, y0=0.0, y1=1.0, u=u, wu=wu, v=v, wv=wv, omega=0.81, mu_ref=0.0, Kn=0.1,
+                   bcs=list(_CHANNEL_BCS), cfl=0.8, steps=10000, name=f"{name}-{nuv}", seed=181008137 + 10 * int(name[1]) + nuv,
+                   eps=(0.01, 0.01, 0.01, 0.01), rho_drop=0.1)
+
+
 def periodic_box(I: int, J: int, Nu: int, Nv: int, a: float = 5.0, Kn: float = 0.1, seed: int = 1,
                  eps=(0.05, 0.05, 0.05, 0.05), lx: float = 1.0, ly: float = 1.0, cfl: float = 0.8,
                  mu_ref: float = 0.0, bu: float | None = None) -> Problem:

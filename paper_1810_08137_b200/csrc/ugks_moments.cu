@@ -378,7 +378,12 @@ static cudaError_t set_attr_cm_all(int smem)
 int setup_moments_attributes(const UgksParams &P)
 {
     if (smem_cm<true>(P) > 227 * 1024) return 1;
-    cudaError_t e = set_attr_cm_all<false>((int)smem_cm<false>(P));
-    if (e == cudaSuccess) e = set_attr_cm_all<true>((int)smem_cm<true>(P));
+    // the attribute is per kernel, not per context: opt every instantiation in to the device maximum once, so that contexts of
+    // different geometries can live side by side
+    static bool done = false;
+    if (done) return 0;
+    cudaError_t e = set_attr_cm_all<false>(227 * 1024);
+    if (e == cudaSuccess) e = set_attr_cm_all<true>(227 * 1024);
+    done = e == cudaSuccess;
     return e == cudaSuccess ? 0 : 1;
 }

@@ -364,9 +364,13 @@ int setup_update_attributes(const UgksParams &P)
 {
     const int s3 = (int)smem_fu(P, 3), s4 = (int)smem_fu(P, 4);
     if (s4 > 227 * 1024) return 1;
-    cudaError_t e = set_attr_sgn<2>(s3);
-    if (e == cudaSuccess) e = set_attr_sgn<1>(s3);
-    if (e == cudaSuccess) e = set_attr_sgn<-1>(s3);
-    if (e == cudaSuccess) e = set_attr_sgn<0>(s4);
+    (void)s3;
+    static bool done = false;                                        // per kernel, not per context: opt in to the device maximum once
+    if (done) return 0;
+    cudaError_t e = set_attr_sgn<2>(227 * 1024);
+    if (e == cudaSuccess) e = set_attr_sgn<1>(227 * 1024);
+    if (e == cudaSuccess) e = set_attr_sgn<-1>(227 * 1024);
+    if (e == cudaSuccess) e = set_attr_sgn<0>(227 * 1024);
+    done = e == cudaSuccess;
     return e == cudaSuccess ? 0 : 1;
 }

@@ -213,3 +213,18 @@ def test_unsorted_and_asymmetric_velocity_nodes():
 def test_paper_meshes_odd_grids_full_field(name, nuv, steps):
     """The paper's own shapes (Table 1): whole-field parity on odd velocity grids with a node at 0."""
     _check(_run_pair(workloads.paper_mesh(name, nuv), steps), max(1, steps) * TOL_1)
+
+
+def test_two_contexts_of_different_geometry_side_by_side():
+    """Contexts with different velocity grids (different shared-memory footprints) stepped alternately."""
+    from oracle import Oracle
+    from paper_1810_08137_b200 import Ugks
+    pa, pb = workloads.channel_config("C4", I=12, J=6), workloads.channel_config("C1", I=10, J=7)
+    (Wa, fa, _), (Wb, fb, _) = workloads.initial_state(pa), workloads.initial_state(pb)
+    ga, gb = Ugks(pa), Ugks(pb)
+    ga.set_state(Wa, fa); gb.set_state(Wb, fb)
+    for _ in range(2):
+        ga.step(1); gb.step(1)
+    for p, W, f, g in ((pa, Wa, fa, ga), (pb, Wb, fb, gb)):
+        o = Oracle(p, threads=4); o.set_state(W, f); o.step(2)
+        assert err_f(g.f(), o.f()) <= 2 * TOL_1 and err_W(g.W(), o.W()) <= 2 * TOL_1

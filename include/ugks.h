@@ -90,7 +90,8 @@ long ugks_step_count(const ugks_ctx *);
 /* Kernels launched by this context since ugks_init (for bench.py's gpu_launches). */
 long ugks_launch_count(const ugks_ctx *);
 /* Tuning knobs: name in {"strip" (cells per CTA march), "chunk_m" (at most that many velocity rows per chunk), "R"
- * (velocity rows processed in parallel by a CTA), "profile" (1: time every kernel of ugks_step with CUDA events)}.
+ * (velocity rows processed in parallel by a CTA), "profile" (1: time every kernel of ugks_step with CUDA events),
+ * "graph" (replay pairs of steps from a CUDA graph: -1 auto = on for launch-bound meshes below 4e6 points, 0 off, 1 on)}.
  * UGKS_EINVAL for unknown names or values that do not fit shared memory / the allocated buffers. */
 int ugks_set_option(ugks_ctx *, const char *name, int value);
 /* With option "profile" on: accumulated device time in ms and launch counts of the five kernels of a step since

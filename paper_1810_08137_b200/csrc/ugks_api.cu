@@ -22,10 +22,16 @@ struct ugks_ctx {
     int profile;              // option "profile": time every kernel of ugks_step with CUDA events
     cudaEvent_t *ev; int nev, nev_used;
     double kms[5]; long kcnt[5];
+    // CUDA graph of two consecutive steps (launch-bound meshes): captured on an internal stream, replayed between two events
+    int graph_mode;           // option "graph": -1 auto (on below 4e6 points per step), 0 off, 1 on
+    int graph_cur;            // parity of the state the graph starts from
+    long graph_launches;      // kernels inside the graph
+    cudaStream_t gst; cudaGraphExec_t gexec; cudaEvent_t gin, gout;
     char err[256];
 };
 
 static char g_err[256] = "";
+extern "C" { static void drop_graph(ugks_ctx *c); }
 static int fail(ugks_ctx *c, int code, const char *fmt, const char *detail)
 {
     char *dst = c ? c->err : g_err;
@@ -175,6 +181,8 @@ static int apply_geometry(ugks_ctx *c, const Chunking *C, int R, int npt, int nc
     for (int i = 0; i < C->n; ++i)
         if ((T.Nu & 1) && (C->c[i].x & 1) && 0) return fail(c, UGKS_EINVAL, "%s", "unaligned chunk");
     CK(cudaStreamSynchronize(c->st), "apply_geometry");
+    if (c->gst) cudaStreamSynchronize(c->gst);
+    drop_graph(c);
     CK(cudaMemcpy(c->chunks_dev, C->c, sizeof(int4) * C->n, cudaMemcpyHostToDevice), "apply_geometry");
     c->P = T;
     if (setup_moments_attributes(c->P) || setup_update_attributes(c->P)) return cuda_fail(c, cudaGetLastError(), "apply_geometry");
@@ -262,6 +270,7 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     memcpy(c->uhost, vg->u, sizeof(double) * vg->Nu);
     c->cells = (size_t)m->I * m->J;
     c->st = (cudaStream_t)cuda_stream;
+    c->graph_mode = -1;
     static Chunking C;
     int R0, npt0;
     choose_geometry(vg->v, P.I, P.J, P.Nu, P.Nv, &C, &R0, &npt0, &P.strip);
@@ -293,6 +302,7 @@ void ugks_destroy(ugks_ctx *c)
 {
     if (!c) return;
     cudaStreamSynchronize(c->st);
+    if (c->gst) { cudaStreamSynchronize(c->gst); drop_graph(c); cudaEventDestroy(c->gin); cudaEventDestroy(c->gout); cudaStreamDestroy(c->gst); }
     for (int i = 0; i < c->nev; ++i) cudaEventDestroy(c->ev[i]);
     free(c->ev);
     free(c->vhost);
@@ -312,6 +322,7 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
     if (!strcmp(name, "strip")) {
         if (value < 1 || value > 4096) return fail(c, UGKS_EINVAL, "%s", "strip out of range");
         P.strip = value;
+        drop_graph(c);
         return UGKS_OK;
     }
     if (!strcmp(name, "chunk_m")) {                                  // re-chunk with at most `value` rows per chunk
@@ -331,6 +342,7 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
         return apply_geometry(c, &C, value, (P.cmax + value - 1) / value, c->nchunk_alloc);
     }
     if (!strcmp(name, "profile")) { c->profile = value != 0; return UGKS_OK; }
+    if (!strcmp(name, "graph")) { c->graph_mode = value < 0 ? -1 : (value != 0); if (!c->graph_mode) drop_graph(c); return UGKS_OK; }
     return fail(c, UGKS_EINVAL, "unknown option %s", name);
 }
 
@@ -358,10 +370,63 @@ int ugks_set_state(ugks_ctx *c, const double *W, const double *f, int on_dev)
     return UGKS_OK;
 }
 
+static void drop_graph(ugks_ctx *c)
+{
+    if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+}
+
+// one step of the five kernels on stream st, from state parity cur; returns the kernels launched
+static long enqueue_step(ugks_ctx *c, int cur, cudaStream_t st)
+{
+    long n = launch_cell_moments(c->P, cur, st);
+    n += launch_face_scalars(c->P, cur, st);
+    n += launch_cell_scalars(c->P, cur, c->resblocks, st);
+    n += launch_tables(c->P, st);
+    n += launch_flux_update(c->P, cur, st);
+    return n;
+}
+
+// replay pairs of steps from a captured graph; returns the steps done (0 if graphs are off or capture is not possible)
+static int step_by_graph(ugks_ctx *c, int n)
+{
+    const bool want = c->graph_mode == 1 || (c->graph_mode < 0 && (double)c->cells * c->P.N < 4.0e6);
+    if (!want || c->profile || n < 4) return 0;
+    if (!c->gst) {
+        if (cudaStreamCreateWithFlags(&c->gst, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->gin, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->gout, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->graph_mode = 0; return 0; }
+    }
+    if (c->gexec && c->graph_cur != c->cur) drop_graph(c);
+    if (!c->gexec) {
+        cudaGraph_t g = nullptr;
+        if (cudaStreamBeginCapture(c->gst, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); c->graph_mode = 0; return 0; }
+        c->graph_launches = enqueue_step(c, c->cur, c->gst) + enqueue_step(c, c->cur ^ 1, c->gst);
+        if (cudaStreamEndCapture(c->gst, &g) != cudaSuccess || !g || cudaGraphInstantiate(&c->gexec, g, 0) != cudaSuccess) {
+            cudaGetLastError(); if (g) cudaGraphDestroy(g); c->gexec = nullptr; c->graph_mode = 0; return 0;
+        }
+        cudaGraphDestroy(g);
+        c->graph_cur = c->cur;
+    }
+    const int pairs = n / 2;
+    cudaEventRecord(c->gin, c->st);
+    cudaStreamWaitEvent(c->gst, c->gin, 0);
+    for (int i = 0; i < pairs; ++i) cudaGraphLaunch(c->gexec, c->gst);
+    cudaEventRecord(c->gout, c->gst);
+    cudaStreamWaitEvent(c->st, c->gout, 0);
+    c->launches += pairs * c->graph_launches;
+    c->steps += 2 * pairs;
+    return 2 * pairs;
+}
+
 int ugks_step(ugks_ctx *c, int n)
 {
     if (!c || n < 0) return fail(c, UGKS_EINVAL, "%s", "bad argument");
     if (!c->have_state) return fail(c, UGKS_ESTATE, "%s", "ugks_step before ugks_set_state");
+    {
+        const int done = step_by_graph(c, n);
+        n -= done;
+        if (done) c->have_res = 1;
+    }
     if (c->profile) {
         const int need = c->nev_used + 6 * n;
         if (need > c->nev) {

@@ -228,3 +228,19 @@ def test_two_contexts_of_different_geometry_side_by_side():
     for p, W, f, g in ((pa, Wa, fa, ga), (pb, Wb, fb, gb)):
         o = Oracle(p, threads=4); o.set_state(W, f); o.step(2)
         assert err_f(g.f(), o.f()) <= 2 * TOL_1 and err_W(g.W(), o.W()) <= 2 * TOL_1
+
+
+def test_graph_replay_matches_plain_launches_bitwise():
+    """ugks_step(n) replays pairs of steps from a CUDA graph on small meshes; the result must be the plain-launch result."""
+    from paper_1810_08137_b200 import Ugks
+    p = workloads.channel_config("C1")
+    W, f, _ = workloads.initial_state(p)
+    outs = []
+    for mode in (0, 1):
+        g = Ugks(p)
+        g.set_option("graph", mode)
+        g.set_state(W, f)
+        g.step(7); g.step(1); g.step(6)                       # odd counts and a parity change between calls
+        outs.append((g.f(), g.W(), g.step_count, g.residual()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert outs[0][2] == outs[1][2] == 14 and np.array_equal(outs[0][3], outs[1][3])

@@ -204,13 +204,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_cell_moments(const UgksParams P,
     const int s3lag = R == 1 ? 1 : 2;                                // pipeline lag of stage 3 behind stage 1
     constexpr int NJ = NC - 6;                                       // stage-2 jobs per column: 3 (x, b = 0..2) + 7 (y) [+ 7]
 
+    int xslot = 2, xphase = 0, ybuf_i = 0, yphase = 0;               // ring slot / phase of row a+1 and of y stage a (a = c0: row c0+1 is the 3rd row)
     for (int a = c0; a < c1 + 3; ++a) {
         if (a < c1) {                                                // stage 1: point sums of cell a
-            wait_x(a + 1);
-            mbar_wait(&bars[NSXM + ((a - c0) & 1)], ((a - c0) >> 1) & 1);
-            const unsigned char *xn = xring_b + ((a + 1 - rows_first) % NSXM) * QbB;
-            const unsigned char *ym = ybuf_b + ((a - c0) & 1) * 2 * QbB, *yp = ym + QbB;
-            const bool xm_miss = beyond_wall<0>(P, a - 1), xp_miss = beyond_wall<0>(P, a + 1);
+            mbar_wait(&bars[xslot], xphase);                         // row a+1
+            mbar_wait(&bars[NSXM + ybuf_i], yphase);
+            const unsigned char *xn = xring_b + xslot * QbB;
+            const unsigned char *ym = ybuf_b + ybuf_i * 2 * QbB, *yp = ym + QbB;
+            if (++xslot == NSXM) { xslot = 0; xphase ^= 1; }
+            if (ybuf_i) yphase ^= 1;
+            ybuf_i ^= 1;
+            const bool xm_miss = a == 0 && P.bc[0] == BC_WALL, xp_miss = a == P.I - 1 && P.bc[1] == BC_WALL;
             double acc[NA];
 #pragma unroll
             for (int i = 0; i < NA; ++i) acc[i] = 0.0;

@@ -19,8 +19,10 @@
  * order are unchanged, so results are bit-identical to the single-thread run).
  * All pointers are HOST pointers.  Every call returns 0 on success, nonzero on error.
  *
- * Parity pins: tests/test_oracle_*.py (P1..P15 of DESIGN.md).  Field values of a
- * full channel step are "parity unpinned" against the paper: PAPER.md prints no
+ * Parity pins: tests/test_oracle_*.py (P1..P15, P17..P19 of DESIGN.md; P17..P19 pin the
+ * equilibrium-slope bracket of S5/S8 and cell_gradW against the exact Euler solution, the
+ * Navier-Stokes shear-wave decay rate and the S5-vs-S8 consistency of every face).  Field
+ * values of a full channel step are "parity unpinned" against the paper: PAPER.md prints no
  * flow-field number (only wall-clock times); they are pinned by invariants instead.
  */
 #ifndef UGKSO_H

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 import workloads
-from tests.util import err_f, err_W
+from tests.util import err_f, err_f_and_tail, err_W
 
 pytestmark = pytest.mark.gpu
 
@@ -32,16 +32,26 @@ def _run_pair(p, steps, W=None, f=None, threads=8):
     g.set_state(W, f)
     o.step(steps)
     g.step(steps)
-    out = dict(ef=err_f(g.f(), o.f()), eW=err_W(g.W(), o.W()), res_g=g.residual(), res_o=o.residual(),
-               Wf_g=g.W_of_f(), Wf_o=o.W_of_f(), g=g, o=o)
-    return out
+    return _compare(g, o)
+
+
+# residual (O11) = sqrt(N_c sum dW^2) / sum |W|: a relative perturbation delta of W moves it by at most ~2 delta in absolute terms,
+# so it is compared at rtol 1e-10 plus 8 x the measured err_W (its conditioning |W| / |dW| grows as the flow converges)
+RES_RTOL = 1e-10
+
+
+def _compare(g, o):
+    ef, tail = err_f_and_tail(g.f(), o.f())
+    return dict(ef=ef, tail=tail, eW=err_W(g.W(), o.W()), res_g=g.residual(), res_o=o.residual(),
+                Wf_g=g.W_of_f(), Wf_o=o.W_of_f(), g=g, o=o)
 
 
 def _check(r, tol):
-    assert r["ef"] <= tol, r["ef"]
-    assert r["eW"] <= tol, r["eW"]
-    assert np.allclose(r["res_g"], r["res_o"], rtol=1e-7, atol=1e-18)
-    assert err_W(r["Wf_g"], r["Wf_o"]) <= tol
+    msg = "err_f %.3e  err_W %.3e  tail (pointwise rel. over f >= 1e-12 cell max) %.3e" % (r["ef"], r["eW"], r["tail"])
+    assert r["ef"] <= tol, msg
+    assert r["eW"] <= tol, msg
+    assert np.all(np.abs(r["res_g"] - r["res_o"]) <= RES_RTOL * np.abs(r["res_o"]) + 8.0 * r["eW"]), (r["res_g"], r["res_o"], msg)
+    assert err_W(r["Wf_g"], r["Wf_o"]) <= tol, msg
 
 
 @pytest.mark.parametrize("steps,tol", [(1, TOL_1), (10, TOL_100), (100, TOL_100)])
@@ -150,18 +160,55 @@ def test_device_pointers_and_errors():
         g.sync()
 
 
-@pytest.mark.parametrize("name", ["C2", "C3", "C5", "C4"])
-def test_full_size_sampled_cells_one_step(name):
-    """BASELINE.json's full sizes in the launch configuration bench.py times (default geometry): one GPU step, then
-    sampled cells (corners, wall rows, inflow/outflow columns, strip seams, interior) against the oracle's one-by-one
-    ``cell_update`` from the same initial state; plus properties that hold at any size (finite, W of the boundary rows)."""
+def _host_ram_or_skip(p, copies, what):
     import psutil
+    need = p.points * 8 * copies
+    if psutil.virtual_memory().available < need:
+        pytest.skip(f"host RAM too small for {what} of {p.name}: {need / 1e9:.0f} GB ({copies} copies of f) needed")
+
+
+# (config, step counts at which the whole field is compared): BASELINE.json's own sizes and step counts (C2 200, C3 100, C5 50,
+# C4 50).  On the 16-core GPU box the oracle needs ~7 s per C4 step, so C4 alone takes ~6 of the suite's ~10 minutes;
+# UGKS_PARITY_C4_STEPS=<n> shortens it.
+_FULL = [("C2", (1, 200)), ("C3", (1, 100)), ("C5", (1, 50)), ("C4", (1, 50))]
+
+
+@pytest.mark.parametrize("name,checkpoints", _FULL)
+def test_full_size_full_field(name, checkpoints):
+    """north_star's acceptance sentence (and P:L136 "identical results ... for the same mesh size"): BASELINE.json's full sizes in
+    the launch configuration bench.py times, the WHOLE field against the oracle run with all host cores: f, W, W_of_f, residual
+    after 1 step (1e-12) and after the config's own step count (1e-10)."""
+    import os
     from oracle import Oracle
     from paper_1810_08137_b200 import Ugks
     p = workloads.channel_config(name)
-    need = p.points * 8 * 3.3
-    if psutil.virtual_memory().available < need:
-        pytest.skip(f"host RAM too small for the oracle state of {name} ({need / 1e9:.0f} GB)")
+    if name == "C4" and os.environ.get("UGKS_PARITY_C4_STEPS"):
+        checkpoints = (1, int(os.environ["UGKS_PARITY_C4_STEPS"]))
+    _host_ram_or_skip(p, 5.5, "the oracle state (2 copies), the input and the two outputs")
+    W, f, _ = workloads.initial_state(p)
+    g = Ugks(p)
+    g.set_state(W, f)
+    o = Oracle(p, threads=os.cpu_count() or 8)
+    o.set_state(W, f)
+    del f
+    done = 0
+    for n in checkpoints:
+        g.step(n - done)
+        o.step(n - done)
+        done = n
+        _check(_compare(g, o), TOL_1 if n == 1 else TOL_100)
+    assert g.step_count == o.step_count == checkpoints[-1]
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C5", "C4"])
+def test_full_size_sampled_cells_one_step(name):
+    """Sampled cells (corners, wall rows, inflow/outflow columns, strip seams, interior) of the full-size configs against the
+    oracle's one-by-one ``cell_update`` from the same initial state -- the check that still runs where the host cannot hold the
+    oracle's whole state; plus properties that hold at any size (finite)."""
+    from oracle import Oracle
+    from paper_1810_08137_b200 import Ugks
+    p = workloads.channel_config(name)
+    _host_ram_or_skip(p, 3.3, "the oracle state")
     W, f, _ = workloads.initial_state(p)
     g = Ugks(p)
     g.set_state(W, f)
@@ -209,7 +256,7 @@ def test_unsorted_and_asymmetric_velocity_nodes():
     _check(_run_pair(q, 3), 3 * TOL_1)
 
 
-@pytest.mark.parametrize("name,nuv,steps", [("M1", 29, 5), ("M2", 49, 1), ("M1", 69, 1)])
+@pytest.mark.parametrize("name,nuv,steps", [("M1", 29, 5), ("M2", 49, 1), ("M1", 69, 1), ("M4", 69, 1), ("M3", 49, 1), ("M4", 29, 10)])
 def test_paper_meshes_odd_grids_full_field(name, nuv, steps):
     """The paper's own shapes (Table 1): whole-field parity on odd velocity grids with a node at 0."""
     _check(_run_pair(workloads.paper_mesh(name, nuv), steps), max(1, steps) * TOL_1)
@@ -240,7 +287,8 @@ def test_graph_replay_matches_plain_launches_bitwise():
         g = Ugks(p)
         g.set_option("graph", mode)
         g.set_state(W, f)
-        g.step(7); g.step(1); g.step(6)                       # odd counts and a parity change between calls
+        g.step(7); g.step(1); g.step(6)                       # odd counts
+        g.step(5); g.step(4)                                  # the second call starts from the other parity: the graph is re-captured
         outs.append((g.f(), g.W(), g.step_count, g.residual()))
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
-    assert outs[0][2] == outs[1][2] == 14 and np.array_equal(outs[0][3], outs[1][3])
+    assert outs[0][2] == outs[1][2] == 23 and np.array_equal(outs[0][3], outs[1][3])

@@ -11,6 +11,23 @@ def err_f(f, f_ref):
     return float(np.max(np.abs(a - b) / scale))
 
 
+def err_f_and_tail(f, f_ref):
+    """(err_f, tail): err_f as above, and the AMB-17 tail metric -- the largest POINTWISE relative error over the points
+    with f_ref >= 1e-12 x (the cell's max f_ref).  Row by row, so that the temporaries stay small at C4 size."""
+    J, I = f_ref.shape[:2]
+    e = t = 0.0
+    for j in range(J):
+        a = f[j].reshape(I, -1)
+        b = f_ref[j].reshape(I, -1)
+        scale = np.max(np.abs(b), axis=1, keepdims=True)
+        d = np.abs(a - b)
+        e = max(e, float(np.max(d / scale)))
+        m = b >= 1e-12 * scale
+        if m.any():
+            t = max(t, float(np.max(d[m] / b[m])))
+    return e, t
+
+
 def err_W(W, W_ref):
     """max |dW_alpha| / S_alpha with S = (rho, rho/sqrt(lam), rho/sqrt(lam), rhoE) of the reference cell."""
     W = W.reshape(-1, 4)

@@ -3,8 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference] [--no-extra]
 
-A "step" is one pass of the whole hot path (face moments x/y, face scalars, cell scalars, flux+update) over the
-synthetic channel workload.  N > 1 (under torchrun) runs N independent replicas ("replicas only": the path is
+A "step" is one pass of the whole hot path (cell moments, face scalars, cell scalars, tables, flux+update) over the
+synthetic channel workload; the default workload is C4, the largest single-GPU configuration of BASELINE.json.  N > 1 (under torchrun) runs N independent replicas ("replicas only": the path is
 single-GPU by north_star); value = points all ranks processed / max-over-ranks device time.
 Prints ONE JSON line on rank 0.  --impl reference times the CPU oracle on a bounded sample instead.
 """
@@ -29,8 +29,50 @@ import workloads  # noqa: E402
 METRIC = "fp64 UGKS cell x velocity-point updates/s"
 UNIT = "updates/s"
 ALG_BYTES_PER_POINT = 16.0          # read f^n once, write f^{n+1} once
-FP64_PER_UPDATE = 85.0              # FP64 instructions per point-update of the built step (from ncu instruction counts)
+DECLARED_BYTES_PER_POINT = 24.0     # the pass structure built: cell_moments reads f (8 B), flux_update reads + writes f (16 B)
+KERNEL_ALG_BYTES = {"cell_moments": 8.0, "flux_update": 16.0}
 FP64_PEAK = 148 * 4 * 16 * 1.965e9  # plain FP64 pipe, thread-instructions/s (one warp DFMA per 2 cycles per sub-partition)
+
+
+def _profile_counts(name):
+    """Per-kernel instruction counts and DRAM traffic of workload ``name`` from the committed ncu capture of this build
+    (profiles/r2_counts.json, written from `ncu --set full` by the command named in profiles/r2_kernels.md): FP64 thread
+    instructions (DFMA + DMUL + DADD, predicated on), all thread instructions, dram bytes -- per launch of one step.
+    None where no capture of that workload is committed (the figures are then reported as null, not guessed)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_counts.json")) as fh:
+            return json.load(fh).get(name)
+    except Exception:
+        return None
+
+
+def _cpu_model():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for ln in fh:
+                if ln.startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def fp64_peak_measured():
+    """thread-level DFMA/s of the plain FP64 pipe, measured by bench_fp64_peak.cu (compiled here with nvcc for sm_100a; a
+    bench-side helper library, not part of libugks)."""
+    import ctypes as C
+    src, so = os.path.join(ROOT, "bench_fp64_peak.cu"), os.path.join(ROOT, "libbench_fp64.so")
+    if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(src):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        tmp = so + f".tmp{os.getpid()}"
+        subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-Xcompiler", "-fPIC", "-shared", "-o", tmp, src], check=True)
+        os.replace(tmp, so)
+    lib = C.CDLL(so)
+    out = C.c_double(0.0)
+    rc = lib.bench_fp64_peak(C.byref(out))
+    if rc:
+        raise RuntimeError(f"bench_fp64_peak -> {rc}")
+    return float(out.value)
 
 
 def _peaks():
@@ -115,12 +157,12 @@ def dist_sum(dist, value, device="cpu"):
     return float(t.item())
 
 
-def oracle_sample(p, seconds_hint=15.0):
+def oracle_sample(p, seconds_hint=15.0, cores=None):
     """The CPU oracle as it stands on a bounded sample of workload p: same physics and velocity grid, the mesh
     cut to the first rows (J_s rows of I cells, walls kept), enough steps for ~10-30 s of CPU work."""
     from oracle import Oracle
-    cores = os.cpu_count() or 1
-    est = 4.0e6 * cores * 0.7                                   # updates/s guess, only to size the sample
+    cores = cores or os.cpu_count() or 1
+    est = 1.0e7 * cores * 0.7                                   # updates/s guess, only to size the sample
     pts_target = est * seconds_hint / 3.0
     Js = int(max(4, min(p.J, pts_target / (p.I * p.N))))
     ps = workloads.channel_config(p.name, I=p.I, J=Js)
@@ -161,8 +203,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * el / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": _workload_name(p), "sample": sample},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "config": {"workload": _workload_name(p) + f" -- timed on the mesh cut {ps.I}x{ps.J} (first {ps.J} rows, walls kept; throughput per point)",
+                       "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "cpu": _cpu_model()},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -175,9 +218,9 @@ def _workload_name(p):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C3", choices=list(workloads.CONFIGS))
+    ap.add_argument("--config", default="C4", choices=list(workloads.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extra", action="store_true", help="skip the other configs / cpu baseline (N=1 default runs them)")
     ap.add_argument("--no-e2e", action="store_true")
@@ -248,44 +291,75 @@ def main():
         return res
 
     p = workloads.channel_config(args.config)
-    from paper_1810_08137_b200 import fp64_peak
-    fp64_measured = fp64_peak()
+    fp64_measured = fp64_peak_measured()
+
+    def hbm_fracs(q, ms_step, kernel_ms):
+        """HBM-roofline fractions of a workload: per f-sized kernel (its algorithmic bytes / its time) and for the step against
+        the 16-B floor and against the declared 24-B pass structure."""
+        out = {"step_frac_of_16B_floor": ALG_BYTES_PER_POINT * q.points / (ms_step * 1e-3) / 1e9 / peak,
+               "step_frac_of_declared_24B": DECLARED_BYTES_PER_POINT * q.points / (ms_step * 1e-3) / 1e9 / peak}
+        for k, bpp in KERNEL_ALG_BYTES.items():
+            gbs = bpp * q.points / (kernel_ms[k] * 1e-3) / 1e9
+            out[k] = {"alg_bytes_per_point": bpp, "achieved_gbs": gbs, "frac": gbs / peak}
+        return out
+
+    def alu_fracs(q, kernel_ms, counts):
+        """FP64-pipe and issue-slot use of the two f-sized kernels from the committed instruction counts and the live times."""
+        if not counts:
+            return None
+        out = {}
+        for k in KERNEL_ALG_BYTES:
+            c = counts.get(k)
+            if not c:
+                continue
+            t = kernel_ms[k] * 1e-3
+            out[k] = {"fp64_inst_per_point": c["fp64_thread_inst"] / q.points, "inst_per_point": c["thread_inst"] / q.points,
+                      "fp64_inst_per_s": c["fp64_thread_inst"] / t, "frac_of_fp64_peak": c["fp64_thread_inst"] / t / fp64_measured,
+                      "dram_bytes": c.get("dram_bytes")}
+        return out
+
     r = measure(p, steps, warmup, e2e=not args.no_e2e, kernels=True)
     value = world * p.points * steps / (r["ms"] * 1e-3)
-    dom = max(r["kernels"], key=lambda k: r["kernels"][k]["ms_per_launch"])
-    share = {k: v["ms_per_launch"] for k, v in r["kernels"].items()}
-    tot = sum(share.values())
-    # bytes the dominant kernel must move per step: flux_update reads f once and writes f once (16 B/pt);
-    # cell_moments reads f once (8 B/pt).  DESIGN.md "Roofline".
-    dom_bytes = (16.0 if dom == "flux_update" else 8.0) * p.points
-    traffic = None                                              # dram bytes of that kernel per step from the committed ncu capture
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            traffic = json.load(fh).get(p.name, {}).get(dom)
-    except Exception:
-        pass
-    achieved = dom_bytes / (r["kernels"][dom]["ms_per_launch"] * 1e-3) / 1e9
+    kms = {k: v["ms_per_launch"] for k, v in r["kernels"].items()}      # per step (a kernel launched once per step and class)
+    tot = sum(kms.values())
+    dom = max(KERNEL_ALG_BYTES, key=lambda k: kms[k])
+    counts = _profile_counts(p.name)
+    alu = alu_fracs(p, kms, counts)
+    hbm = hbm_fracs(p, r["ms"] / steps, kms)
+    # The roof that binds this path is the plain FP64 pipe (and the issue slots that feed it), not HBM (DESIGN.md section 5):
+    # roofline.{achieved, peak, frac} are the dominant kernel's FP64 thread-instructions per second against the measured DFMA
+    # rate; the HBM fractions north_star asks for are in roofline.hbm, for both f-sized kernels and for the step.
+    if alu and dom in alu:
+        roof = {"bound": "alu", "kernel": dom, "achieved": alu[dom]["fp64_inst_per_s"] / 1e12, "peak": fp64_measured / 1e12,
+                "unit": "T FP64 thread-inst/s", "frac": alu[dom]["frac_of_fp64_peak"], "traffic": alu[dom]["dram_bytes"],
+                "peak_source": "measured here: bench_fp64_peak.cu, 8 independent DFMA chains per thread (nominal 148 SMs x 4 x 16 lanes x 1.965 GHz = %.3g)" % FP64_PEAK,
+                "counts_source": "profiles/r2_counts.json (ncu --set full of this build, static per build; times are live)"}
+    else:
+        roof = {"bound": "hbm", "kernel": dom, "achieved": hbm[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": hbm[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                "note": "no committed instruction counts for this workload: HBM fraction of the dominant kernel reported"}
+    roof.update({"hbm": dict(hbm, peak_gbs=peak, peak_source=peak_src), "alu": alu,
+                 "kernel_share_of_step": kms[dom] / tot, "kernel_ms": {k: round(v, 5) for k, v in kms.items()}})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": r["ms"] / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": _workload_name(p), "points_per_step": p.points, "parallelism": f"replicas x{world}",
                        "l2": "inputs larger than L2 (one copy of f = %.0f MB), no flush" % (p.points * 8 / 1e6)
                        if p.points * 8 > 126e6 else "L2-resident workload (f = %.0f MB), no flush" % (p.points * 8 / 1e6)},
-            "clocks": r["clocks"], "gpu_launches": r["launches"],
-            "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                         "fp64": {"peak_thread_dfma_per_s": fp64_measured, "nominal": FP64_PEAK,
-                                  "note": "measured by ugks_fp64_peak (8-chain DFMA kernel); nominal = 148 SMs x 4 x 16 lanes x 1.965 GHz",
-                                  "fp64_inst_per_update": FP64_PER_UPDATE,
-                                  "step_frac_of_fp64_roof": value / world * FP64_PER_UPDATE / fp64_measured},
-                         "kernel_share_of_step": share[dom] / tot,
-                         "kernel_ms": {k: round(v, 5) for k, v in share.items()},
-                         "step_frac_of_16B_floor": ALG_BYTES_PER_POINT * value / world / 1e9 / peak},
-            "e2e": r.get("e2e")}
+            "clocks": r["clocks"], "gpu_launches": r["launches"], "roofline": roof, "e2e": r.get("e2e")}
     if rank == 0 and world == 1 and not args.no_extra:
         v, cores, sample, _ = oracle_sample(p)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        v1, _, sample1, _ = oracle_sample(p, seconds_hint=8.0, cores=1)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "cpu": _cpu_model(),
+                                "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "sample": sample1}}
         others = {}
+
+        def other(q, st, label):
+            rr = measure(q, st, 3, e2e=False, kernels=True)
+            km = {k: v["ms_per_launch"] for k, v in rr["kernels"].items()}
+            others[q.name] = {"value": q.points * st / (rr["ms"] * 1e-3), "ms_per_step": rr["ms"] / st, "steps": st, "workload": label,
+                              "clocks": rr["clocks"], "kernel_ms": {k: round(v, 5) for k, v in km.items()},
+                              "hbm": hbm_fracs(q, rr["ms"] / st, km), "alu": alu_fracs(q, km, _profile_counts(q.name))}
         for name in workloads.CONFIGS:
             if name == args.config or name == "C1":
                 continue
@@ -293,18 +367,10 @@ def main():
             if q.points * 8 * 2.2 > psutil.virtual_memory().available:
                 others[name] = {"skipped": "host RAM too small to stage the input"}
                 continue
-            st = {"C2": 50, "C3": 10, "C4": 4, "C5": 6}[name]
-            rr = measure(q, st, 3, e2e=False, kernels=True)
-            others[name] = {"value": q.points * st / (rr["ms"] * 1e-3), "ms_per_step": rr["ms"] / st, "steps": st,
-                            "workload": _workload_name(q),
-                            "kernel_ms": {k: round(v["ms_per_launch"], 5) for k, v in rr["kernels"].items()},
-                            "step_frac_of_16B_floor": ALG_BYTES_PER_POINT * q.points * st / (rr["ms"] * 1e-3) / 1e9 / peak}
-        for mname, nuv, st in (("M4", 29, 50), ("M4", 69, 20), ("M3", 49, 30)):          # the paper's own shapes (Table 1 / Table 3)
+            other(q, {"C2": 100, "C3": 40, "C4": 20, "C5": 20}[name], _workload_name(q))
+        for mname, nuv, st in (("M4", 29, 100), ("M4", 69, 40), ("M3", 49, 40)):         # the paper's own shapes (Table 1 / Table 3)
             q = workloads.paper_mesh(mname, nuv)
-            rr = measure(q, st, 3, e2e=False, kernels=True)
-            others[q.name] = {"value": q.points * st / (rr["ms"] * 1e-3), "ms_per_step": rr["ms"] / st, "steps": st,
-                              "workload": f"paper mesh {mname} {q.I}x{q.J}, {nuv}x{nuv} velocity grid, Kn=0.1",
-                              "kernel_ms": {k: round(v["ms_per_launch"], 5) for k, v in rr["kernels"].items()}}
+            other(q, st, f"paper mesh {mname} {q.I}x{q.J}, {nuv}x{nuv} velocity grid, Kn=0.1")
         line["other_workloads"] = others
     if rank == 0:
         print(json.dumps(line), flush=True)

@@ -22,6 +22,10 @@
  *     Host copies are enqueued on the context's stream and the call returns after they complete.
  *   - All work is enqueued on the stream given to ugks_init.  ugks_step is asynchronous.
  *   - There is no CPU fallback: without a CUDA device every compute call fails with UGKS_ECUDA.
+ *   - The two kernels that sweep f are compiled by NVRTC at ugks_init with the context's geometry as compile-time constants
+ *     (csrc/ugks_jit_*.cuh, read from the directory of libugks.so); if NVRTC or those sources are missing, ugks_init fails.
+ *   - A context belongs to the device that was current at ugks_init; every call switches to it and back.
+ *   - Calls on different contexts may run concurrently from different host threads; calls on one context may not.
  */
 #ifndef UGKS_H
 #define UGKS_H
@@ -38,7 +42,7 @@ enum { UGKS_BC_PERIODIC = 0, UGKS_BC_FIXED = 1, UGKS_BC_WALL = 2 };
 /* Uniform Cartesian mesh of I x J control volumes.  I, J >= 2. */
 typedef struct { int I, J; double x0, x1, y0, y1; } ugks_mesh;
 /* Discrete velocity grid K x M of the paper = Nu x Nv here.  HOST arrays, copied at init.
- * 1 <= Nu <= 256, Nv >= 1.  Weights must have positive sums. */
+ * 1 <= Nu <= 256 (one thread per column of the velocity grid), 1 <= Nv <= 4096.  Weights must have positive sums. */
 typedef struct { int Nu, Nv; const double *u, *wu, *v, *wv; } ugks_vgrid;
 /* Gas: viscosity exponent omega (mu = mu_ref T^omega), mu_ref (<= 0: derive from Kn, AMB-7),
  * Knudsen number, Prandtl number (must be 1: BGK) and internal degrees of freedom (must be 0). */
@@ -89,18 +93,22 @@ double ugks_mu_ref(const ugks_ctx *);
 long ugks_step_count(const ugks_ctx *);
 /* Kernels launched by this context since ugks_init (for bench.py's gpu_launches). */
 long ugks_launch_count(const ugks_ctx *);
-/* Tuning knobs: name in {"strip" (cells per CTA march), "chunk_m" (at most that many velocity rows per chunk), "R"
+/* Tuning knobs (those that change the launch geometry re-compile the kernels): name in {"strip" (cells per CTA march),
+ * "chunk_m" (at most that many velocity rows per chunk; may only coarsen the default chunking), "R"
  * (velocity rows processed in parallel by a CTA), "profile" (1: time every kernel of ugks_step with CUDA events),
- * "graph" (replay pairs of steps from a CUDA graph: -1 auto = on for launch-bound meshes below 4e6 points, 0 off, 1 on)}.
+ * "graph" (replay pairs of steps from a CUDA graph: -1 auto = on for launch-bound meshes below 4e6 points, 0 off, 1 on),
+ * "poison" (test aid: 1 = NaN-fill the shared memory of every SM before each of the two f-sized kernels)}.
  * UGKS_EINVAL for unknown names or values that do not fit shared memory / the allocated buffers. */
 int ugks_set_option(ugks_ctx *, const char *name, int value);
 /* With option "profile" on: accumulated device time in ms and launch counts of the five kernels of a step since
  * the last call, in launch order: cell_moments, face_scalars, cell_scalars, tables, flux_update.
  * Synchronises the stream and resets the accumulators. */
 int ugks_kernel_times(ugks_ctx *, double ms[5], long counts[5]);
-/* Measured throughput of the plain FP64 pipe: thread-level DFMA per second of a register-resident 8-chain kernel on the
- * current device (the arithmetic roof quoted by bench.py beside the HBM roofline).  Takes ~10 ms. */
-int ugks_fp64_peak(double *thread_dfma_per_s);
+/* Compile the two run-time specialised kernels (k_cell_moments, k_flux_update: NVRTC, sm_100a) for this mesh, velocity grid
+ * and boundary types WITHOUT touching a device: the "does it build" check of a geometry, usable on a machine with no GPU.
+ * log (may be NULL) receives up to log_bytes of the compiler log, including ptxas' per-kernel register / shared-memory lines.
+ * Returns UGKS_OK, UGKS_EINVAL (sizes) or UGKS_ECUDA (compile error: see log). */
+int ugks_jit_check(const ugks_mesh *, const ugks_vgrid *, const ugks_bcs *, char *log, size_t log_bytes);
 const char *ugks_last_error(const ugks_ctx *);           /* library-owned string; ctx may be NULL */
 const char *ugks_version(void);
 void ugks_destroy(ugks_ctx *);

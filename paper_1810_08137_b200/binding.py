@@ -13,7 +13,7 @@ _dp = C.POINTER(C.c_double)
 
 EXPORTS = ["ugks_workspace_bytes", "ugks_init", "ugks_set_state", "ugks_step", "ugks_moments", "ugks_get_f",
            "ugks_residual", "ugks_sync", "ugks_dt", "ugks_mu_ref", "ugks_step_count", "ugks_launch_count",
-           "ugks_set_option", "ugks_kernel_times", "ugks_fp64_peak", "ugks_last_error", "ugks_version", "ugks_destroy"]
+           "ugks_set_option", "ugks_kernel_times", "ugks_jit_check", "ugks_last_error", "ugks_version", "ugks_destroy"]
 
 
 class UgksError(RuntimeError):
@@ -71,7 +71,7 @@ def lib():
         L.ugks_launch_count.argtypes = [vp]; L.ugks_launch_count.restype = C.c_long
         L.ugks_set_option.argtypes = [vp, C.c_char_p, C.c_int]
         L.ugks_kernel_times.argtypes = [vp, _dp, C.POINTER(C.c_long)]
-        L.ugks_fp64_peak.argtypes = [_dp]
+        L.ugks_jit_check.argtypes = [C.POINTER(_Mesh), C.POINTER(_VGrid), C.POINTER(_BCs), C.c_char_p, C.c_size_t]
         L.ugks_last_error.argtypes = [vp]; L.ugks_last_error.restype = C.c_char_p
         L.ugks_version.argtypes = []; L.ugks_version.restype = C.c_char_p
         L.ugks_destroy.argtypes = [vp]; L.ugks_destroy.restype = None
@@ -88,13 +88,15 @@ def _structs(p):
     return keep, mesh, vg, gas, bcs
 
 
-def fp64_peak() -> float:
-    """Measured thread-level DFMA per second of the current device (ugks_fp64_peak)."""
-    out = C.c_double(0.0)
-    rc = lib().ugks_fp64_peak(C.byref(out))
+def jit_check(problem) -> str:
+    """Compile the run-time specialised kernels for ``problem``'s geometry without a device (ugks_jit_check); returns the
+    compiler log (ptxas register / shared-memory lines).  Raises on a compile error."""
+    keep, mesh, vg, gas, bcs = _structs(problem)
+    buf = C.create_string_buffer(1 << 16)
+    rc = lib().ugks_jit_check(C.byref(mesh), C.byref(vg), C.byref(bcs), buf, len(buf))
     if rc:
-        raise UgksError(rc, "ugks_fp64_peak failed")
-    return float(out.value)
+        raise UgksError(rc, buf.value.decode(errors="replace")[-2000:])
+    return buf.value.decode(errors="replace")
 
 
 def workspace_bytes(problem) -> int:

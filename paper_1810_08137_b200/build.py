@@ -47,7 +47,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     from concurrent.futures import ThreadPoolExecutor
     with ThreadPoolExecutor(max_workers=max(1, min(len(sources()), os.cpu_count() or 1))) as ex:
         objs = list(ex.map(compile_one, sources()))
-    subprocess.run([nvcc, *[f for f in flags if f not in ("-lineinfo",)], "-shared", "-o", tmp, *objs], check=True, cwd=CSRC)
+    cuda_lib = os.path.join(os.path.dirname(os.path.dirname(os.path.realpath(nvcc))), "lib64")
+    # NVRTC compiles the two f-sized kernels at ugks_init (csrc/ugks_jit.cu); libnvrtc is found through the rpath
+    link = ["-L" + cuda_lib, "-lnvrtc", "-ldl", "-Xlinker", "-rpath", "-Xlinker", cuda_lib]
+    subprocess.run([nvcc, *[f for f in flags if f not in ("-lineinfo",)], "-shared", "-o", tmp, *objs, *link], check=True, cwd=CSRC)
     os.replace(tmp, SO)
     return SO
 

@@ -1,6 +1,7 @@
 // ugks_api.cu -- the C ABI of include/ugks.h: context, workspace carving, launch sequencing.
 #include "../../include/ugks.h"
 #include "ugks_common.cuh"
+#include "ugks_jit.h"
 
 #include <math.h>
 #include <stdio.h>
@@ -9,6 +10,8 @@
 
 struct ugks_ctx {
     UgksParams P;
+    JitModule *jm;            // run-time specialised k_cell_moments / k_flux_update of this geometry (ugks_jit.cu)
+    int device;               // the device the context was created on; every entry point runs there
     cudaStream_t st;
     int cur;                  // which of f[2] / W[2] holds the current state
     int have_state, have_res;
@@ -17,9 +20,10 @@ struct ugks_ctx {
     double *res_dev, *bcprim_dev, *Wf_dev;
     double *ghost, *wallg, *Wb, *wallG, *ghostmom;   // non-const aliases of the P fields
     int4 *chunks_dev;
-    double *vhost, *uhost;    // host copies of the velocity nodes (chunking, column ranges by sign)
+    double *vhost, *uhost, *wvhost, *wuhost;   // host copies of the velocity nodes and weights (chunking, JIT constants)
     size_t cells;
     int profile;              // option "profile": time every kernel of ugks_step with CUDA events
+    int poison;               // option "poison": NaN-fill every SM's shared memory before each f-sized kernel (test aid)
     cudaEvent_t *ev; int nev, nev_used;
     double kms[5]; long kcnt[5];
     // CUDA graph of two consecutive steps (launch-bound meshes): captured on an internal stream, replayed between two events
@@ -46,6 +50,16 @@ static int cuda_fail(ugks_ctx *c, cudaError_t e, const char *where)
 }
 #define CK(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, where); } while (0)
 
+// every entry point runs on the device the context was created on (function attributes, streams and the workspace live there)
+struct DevGuard {
+    int prev, changed;
+    explicit DevGuard(const ugks_ctx *c) : prev(-1), changed(0)
+    {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) changed = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DevGuard() { if (changed) cudaSetDevice(prev); }
+};
+
 static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 // ---------------------------------------------------------------------------------------------
@@ -54,12 +68,20 @@ static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 // too many runs, everything, go to "mixed" chunks that select the side per point.  Order: [v < 0][v > 0][mixed].
 constexpr int MAXCHUNK = 4096;
 struct Chunking { int n, nneg, npos, nmix, cmax; int4 c[MAXCHUNK]; };
+struct ChunkingBox {             // heap-owned scratch (the table is 64 KB): no static buffers, the ABI is re-entrant
+    Chunking *p;
+    ChunkingBox() : p((Chunking *)calloc(1, sizeof(Chunking))) {}
+    ~ChunkingBox() { free(p); }
+    ChunkingBox(const ChunkingBox &) = delete;
+    ChunkingBox &operator=(const ChunkingBox &) = delete;
+};
 
 static void make_chunks(const double *v, int Nv, int Nu, int cm_target, Chunking *C)
 {
     if (cm_target < 1) cm_target = 1;
     if ((Nu & 1) && (cm_target & 1) && cm_target > 1) cm_target -= 1;
-    int4 tmp[MAXCHUNK];
+    int4 *tmp = (int4 *)malloc(sizeof(int4) * MAXCHUNK);
+    if (!tmp) { C->n = 0; C->cmax = 0; C->nneg = C->npos = C->nmix = 0; return; }
     int nt = 0, nruns = 0;
     bool fallback = false;
     for (int m = 0; m < Nv && !fallback;) {
@@ -76,7 +98,7 @@ static void make_chunks(const double *v, int Nv, int Nu, int cm_target, Chunking
     }
     if (fallback) {
         nt = 0;
-        for (int m = 0; m < Nv; m += cm_target) tmp[nt++] = make_int4(m, (m + cm_target <= Nv ? cm_target : Nv - m), 0, 0);
+        for (int m = 0; m < Nv && nt < MAXCHUNK; m += cm_target) tmp[nt++] = make_int4(m, (m + cm_target <= Nv ? cm_target : Nv - m), 0, 0);
     }
     C->n = 0; C->cmax = 0;
     const int order[3] = { -1, 1, 0 };
@@ -85,6 +107,7 @@ static void make_chunks(const double *v, int Nv, int Nu, int cm_target, Chunking
         for (int i = 0; i < nt; ++i)
             if (tmp[i].z == order[o]) { C->c[C->n++] = tmp[i]; cnt[o]++; if (tmp[i].y > C->cmax) C->cmax = tmp[i].y; }
     C->nneg = cnt[0]; C->npos = cnt[1]; C->nmix = cnt[2];
+    free(tmp);
 }
 
 // R rows in parallel (threads = Nu*R rounded up to a warp multiple), NPT = ceil(cmax / R) <= 7 points per thread:
@@ -121,19 +144,20 @@ struct Layout {
 };
 static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
 {
-    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > 256 || vg->Nv < 1) return 1;
+    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > 256 || vg->Nv < 1 || vg->Nv > MAXCHUNK) return 1;
     const size_t cells = (size_t)m->I * m->J, N = (size_t)vg->Nu * vg->Nv;
     const size_t Npad = (N + 15) & ~(size_t)15;
     const size_t nfx = (size_t)(m->I + 1) * m->J, nfy = (size_t)m->I * (m->J + 1);
     L->NuP = (vg->Nu + 1) & ~1; L->NvP = (vg->Nv + 1) & ~1;
     L->frs = FR_NCOEF + L->NuP + L->NvP; L->crs = CR_NCOEF + 2 * L->NuP + 2 * L->NvP;
-    // the moment buffer holds twice the chunks of the default geometry (room for the "chunk_m" tuning option)
+    // the moment buffer holds the chunks of the default geometry (the "chunk_m" tuning option may only coarsen it)
     if (!vg->v) return 1;
-    static Chunking C;
+    ChunkingBox CB;
+    if (!CB.p) return 1;
     int R, npt, strip;
-    choose_geometry(vg->v, m->I, m->J, vg->Nu, vg->Nv, &C, &R, &npt, &strip);
-    size_t nchunk = 2 * (size_t)C.n;
-    if (nchunk > MAXCHUNK) nchunk = MAXCHUNK;
+    choose_geometry(vg->v, m->I, m->J, vg->Nu, vg->Nv, CB.p, &R, &npt, &strip);
+    size_t nchunk = (size_t)CB.p->n;
+    if (nchunk < 1) return 1;
     L->nchunk_alloc = (int)nchunk;
     L->Npad = (int)Npad;
     L->resblocks = (int)((cells + 127) / 128);
@@ -157,42 +181,72 @@ static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
     return 0;
 }
 
-// install a chunking + (R, npt) in the context: checks buffers and shared memory, uploads the chunk table
+// chunking + (R, npt) + the column ranges by sign of u -> the geometry fields of T; returns a message on failure
+static const char *set_geometry(UgksParams &T, const Chunking *C, int R, int npt, const double *uhost)
+{
+    T.nchunk = C->n; T.nneg = C->nneg; T.npos = C->npos; T.nmix = C->nmix; T.cmax = C->cmax; T.R = R; T.npt = npt;
+    bool sorted = true;                                              // columns by sign of u (sorted nodes)
+    for (int k = 1; k < T.Nu; ++k) if (uhost[k] < uhost[k - 1]) sorted = false;
+    T.kxm_end = T.Nu; T.kxp_begin = 0;
+    if (sorted) {
+        int k0 = 0, k1 = 0;
+        while (k0 < T.Nu && uhost[k0] < 0.0) ++k0;                   // first u >= 0
+        k1 = k0; while (k1 < T.Nu && uhost[k1] <= 0.0) ++k1;         // first u > 0
+        T.kxp_begin = k0; T.kxm_end = k1;
+    }
+    T.s3_nsx = T.s3_nsy = 0;                                         // (the stage-3 split is a compile-time constant of the kernel)
+    if (npt < 1 || npt > 7 || R < 1 || T.Nu * R > 256 || R * npt < C->cmax) return "R / points per thread out of range";
+    if (jit_smem_flux_update(T) > 227 * 1024 || jit_smem_cell_moments(T) > 227 * 1024) return "chunk does not fit in shared memory";
+    return nullptr;
+}
+
+// install a chunking + (R, npt) in the context: checks buffers and shared memory, compiles / fetches the kernels of this
+// geometry, uploads the chunk table
 static int apply_geometry(ugks_ctx *c, const Chunking *C, int R, int npt, int nchunk_alloc)
 {
     UgksParams T = c->P;
-    T.nchunk = C->n; T.nneg = C->nneg; T.npos = C->npos; T.nmix = C->nmix; T.cmax = C->cmax; T.R = R; T.npt = npt;
     if (C->n > nchunk_alloc) return fail(c, UGKS_EINVAL, "%s", "too many chunks for the allocated moment buffer");
-    {   // columns by sign of u (sorted nodes), and the stage-3 split of k_cell_moments
-        bool sorted = true;
-        for (int k = 1; k < T.Nu; ++k) if (c->uhost[k] < c->uhost[k - 1]) sorted = false;
-        T.kxm_end = T.Nu; T.kxp_begin = 0;
-        if (sorted) {
-            int k0 = 0, k1 = 0;
-            while (k0 < T.Nu && c->uhost[k0] < 0.0) ++k0;            // first u >= 0
-            k1 = k0; while (k1 < T.Nu && c->uhost[k1] <= 0.0) ++k1;  // first u > 0
-            T.kxp_begin = k0; T.kxm_end = k1;
-        }
-        const int lenx = T.kxm_end > T.Nu - T.kxp_begin ? T.kxm_end : T.Nu - T.kxp_begin;
-        choose_stage3_split(T.Nu, lenx, (T.Nu * R + 31) / 32 * 32, C->nmix > 0, &T.s3_nsx, &T.s3_nsy);
-    }
-    if (npt < 1 || npt > 7 || R < 1 || T.Nu * R > 256 || R * npt < C->cmax) return fail(c, UGKS_EINVAL, "%s", "R / points per thread out of range");
-    if (smem_flux_update(T) > 227 * 1024 || smem_cell_moments(T) > 227 * 1024) return fail(c, UGKS_EINVAL, "%s", "chunk does not fit in shared memory");
-    for (int i = 0; i < C->n; ++i)
-        if ((T.Nu & 1) && (C->c[i].x & 1) && 0) return fail(c, UGKS_EINVAL, "%s", "unaligned chunk");
+    if (const char *why = set_geometry(T, C, R, npt, c->uhost)) return fail(c, UGKS_EINVAL, "%s", why);
     CK(cudaStreamSynchronize(c->st), "apply_geometry");
     if (c->gst) cudaStreamSynchronize(c->gst);
     drop_graph(c);
+    JitModule *jm = nullptr;
+    char msg[240];
+    if (jit_get(T, C->c, c->uhost, c->wuhost, c->vhost, c->wvhost, &jm, msg, sizeof msg)) return fail(c, UGKS_ECUDA, "%s", msg);
     CK(cudaMemcpy(c->chunks_dev, C->c, sizeof(int4) * C->n, cudaMemcpyHostToDevice), "apply_geometry");
     c->P = T;
-    if (setup_moments_attributes(c->P) || setup_update_attributes(c->P)) return cuda_fail(c, cudaGetLastError(), "apply_geometry");
+    c->jm = jm;
     return UGKS_OK;
 }
 
 extern "C" {
 
-const char *ugks_version(void) { return "ugks-b200 0.1 (sm_100a, fp64)"; }
+const char *ugks_version(void) { return "ugks-b200 0.2 (sm_100a, fp64, NVRTC-specialised kernels)"; }
 const char *ugks_last_error(const ugks_ctx *c) { return c ? c->err : g_err; }
+
+int ugks_jit_check(const ugks_mesh *m, const ugks_vgrid *vg, const ugks_bcs *bcs, char *log, size_t log_bytes)
+{
+    if (log && log_bytes) log[0] = 0;
+    Layout L;
+    if (!bcs || make_layout(m, vg, &L) || !vg->u || !vg->wu || !vg->wv) return fail(nullptr, UGKS_EINVAL, "%s", "invalid mesh or velocity grid");
+    UgksParams T;
+    memset(&T, 0, sizeof T);
+    T.I = m->I; T.J = m->J; T.Nu = vg->Nu; T.Nv = vg->Nv; T.N = vg->Nu * vg->Nv; T.Npad = L.Npad;
+    T.NuP = L.NuP; T.NvP = L.NvP; T.frs = L.frs; T.crs = L.crs;
+    const ugks_bc *b[4] = { &bcs->xmin, &bcs->xmax, &bcs->ymin, &bcs->ymax };
+    for (int s = 0; s < 4; ++s) T.bc[s] = b[s]->type;
+    ChunkingBox CB;
+    if (!CB.p) return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed");
+    int R, npt;
+    choose_geometry(vg->v, T.I, T.J, T.Nu, T.Nv, CB.p, &R, &npt, &T.strip);
+    if (const char *why = set_geometry(T, CB.p, R, npt, vg->u)) return fail(nullptr, UGKS_EINVAL, "%s", why);
+    std::vector<char> cubin;
+    std::string out;
+    const int rc = jit_compile(jit_prelude(T, CB.p->c, vg->u, vg->wu, vg->v, vg->wv), &cubin, &out, true);
+    if (log && log_bytes) snprintf(log, log_bytes, "%s", out.c_str());
+    if (rc) return fail(nullptr, UGKS_ECUDA, "JIT compile failed: %.200s", out.c_str());
+    return UGKS_OK;
+}
 
 size_t ugks_workspace_bytes(const ugks_mesh *m, const ugks_vgrid *vg)
 {
@@ -262,18 +316,19 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     c->chunks_dev = (int4 *)(base + L.chunks); P.chunks = c->chunks_dev;
     c->res_dev = D(L.res); c->bcprim_dev = D(L.bcprim); c->Wf_dev = D(L.Wf);
     c->resblocks = L.resblocks; c->nchunk_alloc = L.nchunk_alloc;
-    c->vhost = (double *)malloc(sizeof(double) * vg->Nv);
+    c->vhost = (double *)malloc(sizeof(double) * 2 * (vg->Nv + vg->Nu));      // one block: v, wv, u, wu
     if (!c->vhost) { free(c); return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed"); }
-    memcpy(c->vhost, vg->v, sizeof(double) * vg->Nv);
-    c->uhost = (double *)malloc(sizeof(double) * vg->Nu);
-    if (!c->uhost) { free(c->vhost); free(c); return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed"); }
-    memcpy(c->uhost, vg->u, sizeof(double) * vg->Nu);
+    c->wvhost = c->vhost + vg->Nv; c->uhost = c->wvhost + vg->Nv; c->wuhost = c->uhost + vg->Nu;
+    memcpy(c->vhost, vg->v, sizeof(double) * vg->Nv); memcpy(c->wvhost, vg->wv, sizeof(double) * vg->Nv);
+    memcpy(c->uhost, vg->u, sizeof(double) * vg->Nu); memcpy(c->wuhost, vg->wu, sizeof(double) * vg->Nu);
     c->cells = (size_t)m->I * m->J;
     c->st = (cudaStream_t)cuda_stream;
     c->graph_mode = -1;
-    static Chunking C;
+    ChunkingBox CB;
+    if (!CB.p) { free(c->vhost); free(c); return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed"); }
     int R0, npt0;
-    choose_geometry(vg->v, P.I, P.J, P.Nu, P.Nv, &C, &R0, &npt0, &P.strip);
+    choose_geometry(vg->v, P.I, P.J, P.Nu, P.Nv, CB.p, &R0, &npt0, &P.strip);
+    if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); free(c->vhost); free(c); return fail(nullptr, UGKS_ECUDA, "%s", "cudaGetDevice failed"); }
 
     double bcprim[16];
     for (int s = 0; s < 4; ++s) { bcprim[s * 4] = b[s]->rho; bcprim[s * 4 + 1] = b[s]->U; bcprim[s * 4 + 2] = b[s]->V; bcprim[s * 4 + 3] = b[s]->T; }
@@ -291,9 +346,9 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     if (e == cudaSuccess) e = cudaMemsetAsync(P.crec, 0, c->cells * (size_t)P.crs * 8, c->st);
     if (e == cudaSuccess) { c->launches += launch_setup(P, c->bcprim_dev, c->ghost, c->wallg, c->Wb, c->wallG, c->ghostmom, c->st); e = cudaGetLastError(); }
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
-    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); free(c->vhost); free(c->uhost); free(c); return rc; }
-    { const int rc = apply_geometry(c, &C, R0, npt0, c->nchunk_alloc);
-      if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); free(c->vhost); free(c->uhost); free(c); return rc; } }
+    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); free(c->vhost); free(c); return rc; }
+    { const int rc = apply_geometry(c, CB.p, R0, npt0, c->nchunk_alloc);
+      if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); free(c->vhost); free(c); return rc; } }
     *out = c;
     return UGKS_OK;
 }
@@ -301,12 +356,12 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
 void ugks_destroy(ugks_ctx *c)
 {
     if (!c) return;
+    DevGuard dg(c);
     cudaStreamSynchronize(c->st);
     if (c->gst) { cudaStreamSynchronize(c->gst); drop_graph(c); cudaEventDestroy(c->gin); cudaEventDestroy(c->gout); cudaStreamDestroy(c->gst); }
     for (int i = 0; i < c->nev; ++i) cudaEventDestroy(c->ev[i]);
     free(c->ev);
     free(c->vhost);
-    free(c->uhost);
     free(c);
 }
 
@@ -317,31 +372,42 @@ long ugks_launch_count(const ugks_ctx *c) { return c ? c->launches : -1; }
 
 int ugks_set_option(ugks_ctx *c, const char *name, int value)
 {
+    DevGuard dg(c);
     if (!c || !name) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     UgksParams &P = c->P;
     if (!strcmp(name, "strip")) {
         if (value < 1 || value > 4096) return fail(c, UGKS_EINVAL, "%s", "strip out of range");
+        ChunkingBox CB;                                              // the strip length is a compile-time constant of the kernels
+        if (!CB.p) return fail(c, UGKS_ENOMEM, "%s", "host allocation failed");
+        CK(cudaStreamSynchronize(c->st), "ugks_set_option");
+        CK(cudaMemcpy(CB.p->c, c->chunks_dev, sizeof(int4) * P.nchunk, cudaMemcpyDeviceToHost), "ugks_set_option");
+        CB.p->n = P.nchunk; CB.p->nneg = P.nneg; CB.p->npos = P.npos; CB.p->nmix = P.nmix; CB.p->cmax = P.cmax;
+        const int old = P.strip;
         P.strip = value;
-        drop_graph(c);
-        return UGKS_OK;
+        const int rc = apply_geometry(c, CB.p, P.R, P.npt, c->nchunk_alloc);
+        if (rc) P.strip = old;
+        return rc;
     }
     if (!strcmp(name, "chunk_m")) {                                  // re-chunk with at most `value` rows per chunk
         if (value < 1 || value > 56) return fail(c, UGKS_EINVAL, "%s", "chunk_m out of range");
-        static Chunking C;
-        make_chunks(c->vhost, P.Nv, P.Nu, value, &C);
+        ChunkingBox CB;
+        if (!CB.p) return fail(c, UGKS_ENOMEM, "%s", "host allocation failed");
+        make_chunks(c->vhost, P.Nv, P.Nu, value, CB.p);
         int R, npt;
-        choose_R(P.Nu, C.cmax, &R, &npt);
-        return apply_geometry(c, &C, R, npt, c->nchunk_alloc);
+        choose_R(P.Nu, CB.p->cmax, &R, &npt);
+        return apply_geometry(c, CB.p, R, npt, c->nchunk_alloc);
     }
     if (!strcmp(name, "R")) {
         if (value < 1 || P.Nu * value > 256) return fail(c, UGKS_EINVAL, "%s", "R out of range");
-        static Chunking C;
+        ChunkingBox CB;
+        if (!CB.p) return fail(c, UGKS_ENOMEM, "%s", "host allocation failed");
         CK(cudaStreamSynchronize(c->st), "ugks_set_option");
-        CK(cudaMemcpy(C.c, c->chunks_dev, sizeof(int4) * P.nchunk, cudaMemcpyDeviceToHost), "ugks_set_option");
-        C.n = P.nchunk; C.nneg = P.nneg; C.npos = P.npos; C.nmix = P.nmix; C.cmax = P.cmax;
-        return apply_geometry(c, &C, value, (P.cmax + value - 1) / value, c->nchunk_alloc);
+        CK(cudaMemcpy(CB.p->c, c->chunks_dev, sizeof(int4) * P.nchunk, cudaMemcpyDeviceToHost), "ugks_set_option");
+        CB.p->n = P.nchunk; CB.p->nneg = P.nneg; CB.p->npos = P.npos; CB.p->nmix = P.nmix; CB.p->cmax = P.cmax;
+        return apply_geometry(c, CB.p, value, (P.cmax + value - 1) / value, c->nchunk_alloc);
     }
     if (!strcmp(name, "profile")) { c->profile = value != 0; return UGKS_OK; }
+    if (!strcmp(name, "poison")) { c->poison = value != 0; drop_graph(c); return UGKS_OK; }
     if (!strcmp(name, "graph")) { c->graph_mode = value < 0 ? -1 : (value != 0); if (!c->graph_mode) drop_graph(c); return UGKS_OK; }
     return fail(c, UGKS_EINVAL, "unknown option %s", name);
 }
@@ -358,6 +424,7 @@ static int check_deferred(ugks_ctx *c, const char *where)
 
 int ugks_set_state(ugks_ctx *c, const double *W, const double *f, int on_dev)
 {
+    DevGuard dg(c);
     if (!c || !W || !f) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     const UgksParams &P = c->P;
     const cudaMemcpyKind kind = on_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
@@ -378,11 +445,14 @@ static void drop_graph(ugks_ctx *c)
 // one step of the five kernels on stream st, from state parity cur; returns the kernels launched
 static long enqueue_step(ugks_ctx *c, int cur, cudaStream_t st)
 {
-    long n = launch_cell_moments(c->P, cur, st);
+    long n = 0;
+    if (c->poison) n += launch_poison_smem(st);
+    n += jit_launch_cell_moments(c->jm, c->P, cur, st);
     n += launch_face_scalars(c->P, cur, st);
     n += launch_cell_scalars(c->P, cur, c->resblocks, st);
     n += launch_tables(c->P, st);
-    n += launch_flux_update(c->P, cur, st);
+    if (c->poison) n += launch_poison_smem(st);
+    n += jit_launch_flux_update(c->jm, c->P, cur, st);
     return n;
 }
 
@@ -408,18 +478,21 @@ static int step_by_graph(ugks_ctx *c, int n)
         c->graph_cur = c->cur;
     }
     const int pairs = n / 2;
-    cudaEventRecord(c->gin, c->st);
-    cudaStreamWaitEvent(c->gst, c->gin, 0);
-    for (int i = 0; i < pairs; ++i) cudaGraphLaunch(c->gexec, c->gst);
-    cudaEventRecord(c->gout, c->gst);
-    cudaStreamWaitEvent(c->st, c->gout, 0);
-    c->launches += pairs * c->graph_launches;
-    c->steps += 2 * pairs;
-    return 2 * pairs;
+    if (cudaEventRecord(c->gin, c->st) != cudaSuccess || cudaStreamWaitEvent(c->gst, c->gin, 0) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int done = 0;
+    for (int i = 0; i < pairs; ++i) {
+        if (cudaGraphLaunch(c->gexec, c->gst) != cudaSuccess) break;      // the error stays pending and surfaces in ugks_step
+        ++done;
+    }
+    if (cudaEventRecord(c->gout, c->gst) == cudaSuccess) cudaStreamWaitEvent(c->st, c->gout, 0);
+    c->launches += done * c->graph_launches;
+    c->steps += 2 * done;
+    return 2 * done;
 }
 
 int ugks_step(ugks_ctx *c, int n)
 {
+    DevGuard dg(c);
     if (!c || n < 0) return fail(c, UGKS_EINVAL, "%s", "bad argument");
     if (!c->have_state) return fail(c, UGKS_ESTATE, "%s", "ugks_step before ugks_set_state");
     {
@@ -439,16 +512,18 @@ int ugks_step(ugks_ctx *c, int n)
     }
     for (int s = 0; s < n; ++s) {
         cudaEvent_t *e = c->profile ? c->ev + c->nev_used : nullptr;
+        if (c->poison) c->launches += launch_poison_smem(c->st);
         if (e) cudaEventRecord(e[0], c->st);
-        c->launches += launch_cell_moments(c->P, c->cur, c->st);       // R, S1, S7 sums (both directions)
+        c->launches += jit_launch_cell_moments(c->jm, c->P, c->cur, c->st);       // R, S1, S7 sums (both directions)
         if (e) cudaEventRecord(e[1], c->st);
         c->launches += launch_face_scalars(c->P, c->cur, c->st);       // S2..S5, wall density
         if (e) cudaEventRecord(e[2], c->st);
         c->launches += launch_cell_scalars(c->P, c->cur, c->resblocks, c->st);   // U1, U2 scalars, residual partials
         if (e) cudaEventRecord(e[3], c->st);
         c->launches += launch_tables(c->P, c->st);                     // S6 / U2 separable Maxwellian factors
+        if (c->poison) c->launches += launch_poison_smem(c->st);
         if (e) cudaEventRecord(e[4], c->st);
-        c->launches += launch_flux_update(c->P, c->cur, c->st);        // R, S6, S8, U3
+        c->launches += jit_launch_flux_update(c->jm, c->P, c->cur, c->st);        // R, S6, S8, U3
         if (e) { cudaEventRecord(e[5], c->st); c->nev_used += 6; }
         c->cur ^= 1;
         c->steps += 1;
@@ -460,6 +535,7 @@ int ugks_step(ugks_ctx *c, int n)
 
 int ugks_kernel_times(ugks_ctx *c, double ms[5], long counts[5])
 {
+    DevGuard dg(c);
     if (!c || !ms || !counts) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     CK(cudaStreamSynchronize(c->st), "ugks_kernel_times");
     for (int i = 0; i + 5 < c->nev_used; i += 6)
@@ -475,12 +551,14 @@ int ugks_kernel_times(ugks_ctx *c, double ms[5], long counts[5])
 
 int ugks_sync(ugks_ctx *c)
 {
+    DevGuard dg(c);
     if (!c) return fail(c, UGKS_EINVAL, "%s", "NULL context");
     return check_deferred(c, "ugks_sync");
 }
 
 int ugks_moments(ugks_ctx *c, double *W_stored, double *W_of_f, int on_dev)
 {
+    DevGuard dg(c);
     if (!c) return fail(c, UGKS_EINVAL, "%s", "NULL context");
     if (!c->have_state) return fail(c, UGKS_ESTATE, "%s", "no state");
     const UgksParams &P = c->P;
@@ -496,6 +574,7 @@ int ugks_moments(ugks_ctx *c, double *W_stored, double *W_of_f, int on_dev)
 
 int ugks_get_f(ugks_ctx *c, double *f, int on_dev)
 {
+    DevGuard dg(c);
     if (!c || !f) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     if (!c->have_state) return fail(c, UGKS_ESTATE, "%s", "no state");
     const UgksParams &P = c->P;
@@ -506,6 +585,7 @@ int ugks_get_f(ugks_ctx *c, double *f, int on_dev)
 
 int ugks_residual(ugks_ctx *c, double res[4])
 {
+    DevGuard dg(c);
     if (!c || !res) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     if (!c->have_res) return fail(c, UGKS_ESTATE, "%s", "ugks_residual before the first step");
     c->launches += launch_residual_final(c->P, c->resblocks, c->res_dev, c->st);

@@ -65,7 +65,7 @@ struct UgksParams {
     int R;                           // velocity rows processed in parallel by one CTA (threads = Nu*R rounded up to 32)
     int npt;                         // velocity points per thread = ceil(cmax / R), 1..7 (template parameter)
     int kxm_end, kxp_begin;          // columns with u_k <= 0 are [0, kxm_end), with u_k >= 0 [kxp_begin, Nu) (sorted nodes; else 0..Nu)
-    int s3_nsx, s3_nsy;              // k_cell_moments stage 3: parts per x-output / y-output dot product
+    int s3_nsx, s3_nsy;              // unused (the stage-3 split of k_cell_moments is a compile-time constant)
 };
 
 static __host__ __device__ inline int nfaces_x(const UgksParams &P) { return (P.I + 1) * P.J; }
@@ -169,18 +169,13 @@ __device__ __forceinline__ double warp_sum(double x)
     return x;
 }
 
-// launchers (one per translation unit); each returns the number of kernels it enqueued
-int launch_cell_moments(const UgksParams &P, int cur, cudaStream_t st);
+// launchers of the O(faces) / O(cells) kernels (ugks_scalars.cu); each returns the number of kernels it enqueued.  The two
+// f-sized kernels are compiled at run time and launched through ugks_jit.h.
 int launch_face_scalars(const UgksParams &P, int cur, cudaStream_t st);
 int launch_cell_scalars(const UgksParams &P, int cur, int resblocks, cudaStream_t st);
 int launch_tables(const UgksParams &P, cudaStream_t st);
-int launch_flux_update(const UgksParams &P, int cur, cudaStream_t st);
 int launch_setup(const UgksParams &P, const double *bc_prims /*dev [4][4]*/, double *ghost, double *wallg,
                  double *Wb, double *wallG, double *ghostmom, cudaStream_t st);
 int launch_residual_final(const UgksParams &P, int resblocks, double *res_dev, cudaStream_t st);
 int launch_moments_of_f(const UgksParams &P, const double *f, double *Wf, cudaStream_t st);
-int setup_moments_attributes(const UgksParams &P);
-int setup_update_attributes(const UgksParams &P);
-size_t smem_cell_moments(const UgksParams &P);
-void choose_stage3_split(int Nu, int lenx, int B, bool any_mixed, int *nsx, int *nsy);
-size_t smem_flux_update(const UgksParams &P);
+int launch_poison_smem(cudaStream_t st);

@@ -1,0 +1,215 @@
+// ugks_jit.cu -- run-time specialisation of the two f-sized kernels (k_cell_moments, k_flux_update).
+//
+// ugks_init (and every option that changes the launch geometry) generates a prelude of compile-time constants -- mesh and
+// velocity-grid sizes, boundary types, chunk table, R / NPT / strip, the velocity nodes and weights as hexadecimal literals --
+// and compiles csrc/ugks_jit_moments.cuh + csrc/ugks_jit_update.cuh with NVRTC for sm_100a (-lineinfo).  The cubin is loaded
+// through the runtime's library API (cudaLibraryLoadData / cudaLibraryGetKernel); compiled modules are cached per process by
+// their prelude, so contexts of equal geometry share one module.  There is no other path: if NVRTC or the sources are missing,
+// ugks_init fails.
+#include "ugks_common.cuh"
+#include "ugks_jit.h"
+
+#include <dlfcn.h>
+#include <nvrtc.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <map>
+#include <mutex>
+#include <string>
+#include <vector>
+
+namespace {
+
+std::mutex g_mu;
+std::map<std::string, JitModule *> g_cache;
+
+int pad2i(int x) { return (x + 1) & ~1; }
+int cdivi(int a, int b) { return (a + b - 1) / b; }
+
+// host mirrors of MomL<MIXED>::BYTES and StageL<NY>::BYTES (the device code static_asserts that they agree)
+int smem_mom(const UgksParams &P, bool mixed)
+{
+    const int BT = (P.Nu * P.R + 31) / 32 * 32, QB = pad2i(P.cmax * P.Nu + 1);
+    const int NA = mixed ? 20 : 13, NC = mixed ? 23 : 16, ny = mixed ? 26 : 13;
+    const int lenx = P.kxm_end > P.Nu - P.kxp_begin ? P.kxm_end : P.Nu - P.kxp_begin;
+    int per = P.Nu;
+    for (int q = 1; q <= P.Nu; ++q) if (26 * cdivi(lenx, q) + ny * cdivi(P.Nu, q) <= BT) { per = q; break; }
+    const int nitem = 26 * cdivi(lenx, per) + ny * cdivi(P.Nu, per), NUS = P.Nu | 1, NROW = P.R * P.npt + 1;
+    const int total = 3 * QB + 4 * QB + (P.R == 1 ? 0 : 2 * NA * BT) + pad2i(2 * NC * NUS) + pad2i(13 * NUS) + pad2i(NROW * 6) +
+                      pad2i(2 * nitem) + 5;
+    return total * 8;
+}
+int smem_upd(const UgksParams &P, int ny)
+{
+    const int QB = pad2i(P.cmax * P.Nu + 1), CMP = pad2i(P.cmax + 1);
+    const int size = ny * QB + 3 * (FR_NCOEF + P.NuP) + 3 * CMP + (CR_NCOEF + 2 * P.NuP) + 2 * CMP;
+    return (3 * QB + 2 * size) * 8 + 5 * 8;
+}
+// CTAs per SM for __launch_bounds__: what shared memory allows, capped so that a thread keeps at least `regs` registers
+int min_blocks(int threads, int smem, int regs)
+{
+    int by_smem = (227 * 1024) / (smem + 1024);
+    int by_regs = 65536 / (threads * regs);
+    int b = by_smem < by_regs ? by_smem : by_regs;
+    return b < 1 ? 1 : (b > 16 ? 16 : b);
+}
+
+std::string dir_of_this_library()
+{
+    Dl_info info;
+    if (!dladdr((const void *)&jit_smem_cell_moments, &info) || !info.dli_fname) return ".";
+    std::string p(info.dli_fname);
+    const size_t s = p.rfind('/');
+    return s == std::string::npos ? "." : p.substr(0, s);
+}
+bool read_file(const std::string &path, std::string *out)
+{
+    FILE *f = fopen(path.c_str(), "rb");
+    if (!f) return false;
+    char buf[1 << 14];
+    size_t n;
+    out->clear();
+    while ((n = fread(buf, 1, sizeof buf, f)) > 0) out->append(buf, n);
+    fclose(f);
+    return true;
+}
+
+void add_doubles(std::string &s, const char *name, const double *a, int n)
+{
+    char buf[64];
+    s += "__constant__ double "; s += name; s += "[] = {";
+    for (int i = 0; i < n; ++i) { snprintf(buf, sizeof buf, "%s%a", i ? ", " : "", a[i]); s += buf; }
+    s += "};\n";
+}
+
+}  // namespace
+
+size_t jit_smem_cell_moments(const UgksParams &P) { return (size_t)smem_mom(P, P.nmix > 0); }
+size_t jit_smem_flux_update(const UgksParams &P) { return (size_t)smem_upd(P, P.nmix > 0 ? 4 : 3); }
+
+std::string jit_prelude(const UgksParams &P, const int4 *chunks, const double *u, const double *wu, const double *v, const double *wv)
+{
+    const int threads = (P.Nu * P.R + 31) / 32 * 32 + 32;
+    const int sm_u = smem_mom(P, false), sm_m = smem_mom(P, true), su3 = smem_upd(P, 3), su4 = smem_upd(P, 4);
+    std::string s;
+    char b[256];
+#define DEF(name, val) do { snprintf(b, sizeof b, "#define %s %d\n", name, (int)(val)); s += b; } while (0)
+    DEF("G_I", P.I); DEF("G_J", P.J); DEF("G_NU", P.Nu); DEF("G_NV", P.Nv); DEF("G_NPAD", P.Npad); DEF("G_NUP", P.NuP); DEF("G_NVP", P.NvP);
+    DEF("G_FRS", P.frs); DEF("G_CRS", P.crs);
+    DEF("G_BC0", P.bc[0]); DEF("G_BC1", P.bc[1]); DEF("G_BC2", P.bc[2]); DEF("G_BC3", P.bc[3]);
+    DEF("G_NCHUNK", P.nchunk); DEF("G_NMIX", P.nmix); DEF("G_MC", P.cmax); DEF("G_R", P.R); DEF("G_NPT", P.npt); DEF("G_STRIP", P.strip);
+    DEF("G_KXM_END", P.kxm_end); DEF("G_KXP_BEGIN", P.kxp_begin);
+    { int ragged = 0; for (int i = 0; i < P.nchunk; ++i) if (chunks[i].y != P.cmax) ragged = 1; DEF("G_RAGGED", ragged); }
+    DEF("G_SMEM_MOM", sm_u); DEF("G_SMEM_MOMX", sm_m); DEF("G_SMEM_UPD3", su3); DEF("G_SMEM_UPD4", su4);
+    DEF("G_MINB_MOM", min_blocks(threads, sm_u, 128)); DEF("G_MINB_MOMX", min_blocks(threads, sm_m, 128));
+    DEF("G_MINB_UPD", min_blocks(threads, P.nmix > 0 ? su4 : su3, 128));
+#undef DEF
+    s += "__constant__ int4 c_chunks[] = {";
+    for (int i = 0; i < P.nchunk; ++i) { snprintf(b, sizeof b, "%s{%d, %d, %d, 0}", i ? ", " : "", chunks[i].x, chunks[i].y, chunks[i].z); s += b; }
+    s += "};\n";
+    if (const char *extra = getenv("UGKS_JIT_DEFS")) { s += extra; s += "\n"; }      // developer aid: extra #define lines for experiments
+    add_doubles(s, "c_u", u, P.Nu); add_doubles(s, "c_wu", wu, P.Nu); add_doubles(s, "c_v", v, P.Nv); add_doubles(s, "c_wv", wv, P.Nv);
+    return s;
+}
+
+// compile (no device needed).  On success *cubin holds the image; log receives the NVRTC log (ptxas -v lines with verbose).
+int jit_compile(const std::string &prelude, std::vector<char> *cubin, std::string *log, bool verbose)
+{
+    static const char *names[3] = { "ugks_jit_common.cuh", "ugks_jit_moments.cuh", "ugks_jit_update.cuh" };
+    const std::string dir = dir_of_this_library() + "/csrc/";
+    std::string hdr[3];
+    for (int i = 0; i < 3; ++i)
+        if (!read_file(dir + names[i], &hdr[i])) { *log = "cannot read " + dir + names[i]; return 1; }
+    const std::string src = prelude + "#include \"ugks_jit_moments.cuh\"\n#include \"ugks_jit_update.cuh\"\n";
+    const char *hsrc[3] = { hdr[0].c_str(), hdr[1].c_str(), hdr[2].c_str() };
+    nvrtcProgram prog;
+    if (nvrtcCreateProgram(&prog, src.c_str(), (dir + "ugks_jit_generated.cu").c_str(), 3, hsrc, names) != NVRTC_SUCCESS) { *log = "nvrtcCreateProgram failed"; return 1; }
+    std::vector<const char *> opts = { "--gpu-architecture=sm_100a", "-lineinfo", "--std=c++17", "-default-device" };
+    if (verbose) opts.push_back("--ptxas-options=-v");
+    const nvrtcResult rc = nvrtcCompileProgram(prog, (int)opts.size(), opts.data());
+    size_t n = 0;
+    nvrtcGetProgramLogSize(prog, &n);
+    log->assign(n, '\0');
+    if (n) nvrtcGetProgramLog(prog, &(*log)[0]);
+    if (rc != NVRTC_SUCCESS) { nvrtcDestroyProgram(&prog); *log = std::string("NVRTC: ") + nvrtcGetErrorString(rc) + "\n" + *log; return 1; }
+    nvrtcGetCUBINSize(prog, &n);
+    cubin->resize(n);
+    nvrtcGetCUBIN(prog, cubin->data());
+    nvrtcDestroyProgram(&prog);
+    if (const char *dump = getenv("UGKS_JIT_DUMP")) {               // developer aid: keep the image for cuobjdump -sass
+        if (FILE *f = fopen(dump, "wb")) { fwrite(cubin->data(), 1, cubin->size(), f); fclose(f); }
+    }
+    return n ? 0 : 1;
+}
+
+int jit_get(const UgksParams &P, const int4 *chunks, const double *u, const double *wu, const double *v, const double *wv,
+            JitModule **out, char *err, size_t errlen)
+{
+    const std::string pre = jit_prelude(P, chunks, u, wu, v, wv);
+    std::lock_guard<std::mutex> lock(g_mu);
+    JitModule *m = nullptr;
+    auto it = g_cache.find(pre);
+    if (it != g_cache.end()) m = it->second;
+    else {
+        std::vector<char> cubin;
+        std::string log;
+        if (jit_compile(pre, &cubin, &log, false)) { snprintf(err, errlen, "JIT compile failed: %.200s", log.c_str()); return 1; }
+        m = new JitModule();
+        m->image.swap(cubin);
+        cudaError_t e = cudaLibraryLoadData(&m->lib, m->image.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+        if (e == cudaSuccess) e = cudaLibraryGetKernel(&m->k_mom, m->lib, "k_cell_moments");
+        if (e == cudaSuccess) e = cudaLibraryGetKernel(&m->k_upd, m->lib, "k_flux_update");
+        if (e == cudaSuccess && P.nmix > 0) e = cudaLibraryGetKernel(&m->k_momx, m->lib, "k_cell_moments_mixed");
+        if (e != cudaSuccess) { snprintf(err, errlen, "JIT load failed: %s", cudaGetErrorString(e)); delete m; return 1; }
+        m->threads = (P.Nu * P.R + 31) / 32 * 32 + 32;
+        m->smem_mom = smem_mom(P, false); m->smem_momx = smem_mom(P, true); m->smem_upd = smem_upd(P, P.nmix > 0 ? 4 : 3);
+        g_cache[pre] = m;
+    }
+    // shared-memory opt-in: a function attribute of the CURRENT device, set for every context (cheap, idempotent)
+    cudaError_t e = cudaFuncSetAttribute((const void *)m->k_mom, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem_mom);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)m->k_upd, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem_upd);
+    if (e == cudaSuccess && P.nmix > 0) e = cudaFuncSetAttribute((const void *)m->k_momx, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem_momx);
+    if (e != cudaSuccess) { snprintf(err, errlen, "shared-memory opt-in failed: %s", cudaGetErrorString(e)); return 1; }
+    *out = m;
+    return 0;
+}
+
+static KArgs_h make_args(const UgksParams &P, int cur)
+{
+    KArgs_h a;
+    a.fcur = P.f[cur]; a.fnew = P.f[cur ^ 1]; a.cmom = P.cmom; a.frec0 = P.frec[0]; a.frec1 = P.frec[1]; a.crec = P.crec;
+    a.ghost = P.ghost; a.wallg = P.wallg;
+    return a;
+}
+
+int jit_launch_cell_moments(const JitModule *m, const UgksParams &P, int cur, cudaStream_t st)
+{
+    const int nstrip = (P.I + P.strip - 1) / P.strip;
+    KArgs_h a = make_args(P, cur);
+    int n = 0;
+    if (P.nneg + P.npos) {
+        int chunk0 = 0;
+        void *args[2] = { &a, &chunk0 };
+        cudaLaunchKernel((const void *)m->k_mom, dim3(P.J * nstrip * (P.nneg + P.npos)), dim3(m->threads), args, m->smem_mom, st);
+        ++n;
+    }
+    if (P.nmix) {
+        int chunk0 = P.nneg + P.npos;
+        void *args[2] = { &a, &chunk0 };
+        cudaLaunchKernel((const void *)m->k_momx, dim3(P.J * nstrip * P.nmix), dim3(m->threads), args, m->smem_momx, st);
+        ++n;
+    }
+    return n;
+}
+
+int jit_launch_flux_update(const JitModule *m, const UgksParams &P, int cur, cudaStream_t st)
+{
+    const int nstrip = (P.I + P.strip - 1) / P.strip;
+    KArgs_h a = make_args(P, cur);
+    int chunk0 = 0;
+    void *args[2] = { &a, &chunk0 };
+    cudaLaunchKernel((const void *)m->k_upd, dim3(P.J * nstrip * P.nchunk), dim3(m->threads), args, m->smem_upd, st);
+    return 1;
+}

@@ -1,0 +1,298 @@
+// ugks_jit_update.cuh -- k_flux_update: S6 + S8 at the four faces of every cell fused with the update U3
+// (Eq. (3)); the per-face coefficients (S2..S5), the per-cell relaxation scalars (U1/U2) and every exponential
+// come precomputed from k_face_scalars / k_cell_scalars / k_tables.  Compiled by NVRTC per context (ugks_jit_common.cuh).
+//
+// One CTA marches along a strip of cells of row j for one chunk of velocity rows (all v_m of one sign where the grid
+// allows: SGN = +1 / -1; SGN = 0 is the generic per-point path).  Thread (k, r) owns velocity column k and the rows
+// m = r + p*R.  Step a evaluates x-face a and then finishes cell a-1.
+//   * everything that depends on the face and on u_k only is formed once per face per thread: the four coefficients of the
+//     flux polynomial in the other velocity (already multiplied by the separable Maxwellian factor of u_k) and the two
+//     coefficients of f0 and h sigma0.  Per point that leaves a cubic (Horner), one table factor and two FMAs per face.
+//   * x-stencil: the two older rows of each thread's window live in registers; ONE new row per step comes from a 3-slot
+//     shared-memory ring fed by 1-D TMA bulk copies.  The x-face flux is evaluated once per face and carried in registers to
+//     the next cell.
+//   * y-stencil: three rows ((j-2, j-1, j+1) for v > 0, (j-1, j+1, j+2) for v < 0) are TMA-staged per cell, double-buffered,
+//     together with the records of the step (face and cell coefficients, separable factors).
+//   * f^{n+1} is written straight from registers: f crosses HBM once each way in this kernel.
+#pragma once
+#include "ugks_jit_common.cuh"
+
+constexpr int NSX = 3;                                               // x-ring slots: rows a, a+1 live, a+2 in flight
+constexpr int CMP = pad2c(MC + 1);                                   // doubles per staged piece of a per-row (m) table
+
+template <int NY>
+struct StageL {                                                      // offsets in doubles inside one step stage
+    static constexpr int yrow = 0;
+    static constexpr int xrec = yrow + NY * QB;
+    static constexpr int xm = xrec + FR_NCOEF + NUP;
+    static constexpr int ylrec = xm + CMP;
+    static constexpr int ylm = ylrec + FR_NCOEF + NUP;
+    static constexpr int yurec = ylm + CMP;
+    static constexpr int yum = yurec + FR_NCOEF + NUP;
+    static constexpr int crec = yum + CMP;
+    static constexpr int cgn = crec + CR_NCOEF + 2 * NUP;
+    static constexpr int cgp = cgn + CMP;
+    static constexpr int size = cgp + CMP;
+    static constexpr int BYTES = (NSX * QB + 2 * size) * 8 + (NSX + 2) * 8;
+};
+
+template <int SGN>
+__device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, const int j, const int s)
+{
+    constexpr int NY = SGN == 0 ? 4 : 3;
+    using L = StageL<NY>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int c0 = s * STRIP, c1 = min(c0 + STRIP, GI);              // cells [c0, c1) of row j
+    const int m0 = ch.x, mc = ch.y;
+    const int q0 = m0 * NU, qa = q0 & ~1, qsh = q0 - qa;
+    const int ma = m0 & ~1, msh = m0 - ma;
+    const uint32_t bytes = (uint32_t)(pad2c(mc * NU + qsh) * 8);
+    const uint32_t mbytes = (uint32_t)(pad2c(mc + msh) * 8);
+    constexpr uint32_t kbytes = (FR_NCOEF + NUP) * 8, cbytes = (CR_NCOEF + 2 * NUP) * 8;
+
+    double *ring = reinterpret_cast<double *>(smem_raw);             // [NSX][QB]
+    double *stages = ring + NSX * QB;                                // [2][L::size]
+    uint64_t *bars = reinterpret_cast<uint64_t *>(stages + 2 * L::size);   // [NSX] x rows, [2] stages
+
+    const int tid = threadIdx.x;
+    const bool active = tid < NU * R;
+    const int k = active ? tid % NU : 0, r = active ? tid / NU : 0;
+    const double *fcur = A.fcur;
+    const int rows_first = c0 - 2, rows_last = c1 + 1;
+    if (tid >= BT) {                                                 // ---- producer warp: one lane issues every bulk copy
+        const bool lead = tid == BT;
+        // global sources of a step, linear in the cell index: y-neighbour rows, face records, cell records
+        const int djs[4] = { SGN == 0 ? -2 : (SGN > 0 ? -2 : -1), SGN == 0 ? -1 : (SGN > 0 ? -1 : 1), SGN == 0 ? 1 : (SGN > 0 ? 1 : 2), 2 };
+        const double *yb[NY];
+        int yst[NY];
+#pragma unroll
+        for (int d = 0; d < NY; ++d) yb[d] = yrow_base(fcur, A.ghost, j + djs[d], &yst[d]) + qa;
+        const double *xrp = A.frec0 + (size_t)j * (GI + 1) * FRS;
+        const double *ylp = A.frec1 + (size_t)j * GI * FRS, *yup = ylp + (size_t)GI * FRS;
+        const double *crp = A.crec + (size_t)j * GI * CRS;
+        const int moffK = FR_NCOEF + NUP + ma, moffC = CR_NCOEF + 2 * NUP + ma;
+
+        auto issue_x = [&](int row) {
+            const int sl = (row - rows_first) % NSX;
+            mbar_expect_tx(&bars[sl], bytes);
+            tma_load_1d(ring + sl * QB, xrow_ptr(fcur, A.ghost, row, j) + qa, bytes, &bars[sl]);
+        };
+        // stage of step st: record of x-face st and, for cell st-1, its y-neighbour rows, y-face records and cell record
+        auto issue_stage = [&](int st) {
+            const int sl = (st - c0) & 1;
+            double *S = stages + sl * L::size;
+            uint64_t *bar = &bars[NSX + sl];
+            const bool have_cell = st > c0;
+            mbar_expect_tx(bar, kbytes + mbytes + (have_cell ? NY * bytes + 2 * (kbytes + mbytes) + cbytes + 2 * mbytes : 0));
+            const double *xr = xrp + (size_t)st * FRS;
+            tma_load_1d(S + L::xrec, xr, kbytes, bar);
+            tma_load_1d(S + L::xm, xr + moffK, mbytes, bar);
+            if (have_cell) {
+                const size_t cell = st - 1;
+#pragma unroll
+                for (int d = 0; d < NY; ++d) tma_load_1d(S + L::yrow + d * QB, yb[d] + cell * yst[d], bytes, bar);
+                const double *yl = ylp + cell * FRS, *yu = yup + cell * FRS, *cr = crp + cell * CRS;
+                tma_load_1d(S + L::ylrec, yl, kbytes, bar);
+                tma_load_1d(S + L::ylm, yl + moffK, mbytes, bar);
+                tma_load_1d(S + L::yurec, yu, kbytes, bar);
+                tma_load_1d(S + L::yum, yu + moffK, mbytes, bar);
+                tma_load_1d(S + L::crec, cr, cbytes, bar);
+                tma_load_1d(S + L::cgn, cr + moffC, mbytes, bar);
+                tma_load_1d(S + L::cgp, cr + moffC + NVP, mbytes, bar);
+            }
+        };
+
+        if (lead) {
+            for (int i = 0; i < NSX + 2; ++i) mbar_init(&bars[i], 1);
+            mbar_fence_init();
+        }
+        __syncthreads();
+        if (lead) {
+            for (int row = rows_first; row < rows_first + NSX; ++row) issue_x(row);
+            issue_stage(c0);
+            issue_stage(c0 + 1);
+        }
+        __syncthreads();                                             // rows c0-2, c0-1 consumed
+        if (lead) { issue_x(c0 + 1); issue_x(c0 + 2); }
+        for (int a = c0; a <= c1; ++a) {
+            __syncthreads();                                         // step a done: row a and stage a are free
+            if (lead) {
+                if (a + 3 <= rows_last) issue_x(a + 3);
+                if (a + 2 <= c1) issue_stage(a + 2);
+            }
+        }
+        return;
+    }
+    __syncthreads();                                                 // barriers initialised
+
+    const double uk = c_u[k];
+    const bool posx = uk > 0.0;
+    const double sgx = posx ? 1.0 : -1.0;
+    // Per-thread points p: velocity row m = r + p R; byte offsets are thread base + immediates.  A point outside the chunk
+    // (the last point when R*NPT > MC, the tail of a ragged chunk) re-reads the chunk's first element; only its store is masked.
+    constexpr int QSTEP = R * NU * 8, MSTEP = R * 8;
+    const int qb0 = (qsh + r * NU + k) * 8, mb0 = (msh + r) * 8;
+    int qo[NPT], mo[NPT];
+#pragma unroll
+    for (int p = 0; p < NPT; ++p) { qo[p] = r + p * R < mc ? p * QSTEP : qsh * 8 - qb0; mo[p] = r + p * R < mc ? p * MSTEP : msh * 8 - mb0; }
+#define QOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * QSTEP : qo[p])
+#define MOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * MSTEP : mo[p])
+    double vn[NPT], fm[NPT], fc[NPT], Fprev[NPT];
+    bool valid[NPT];
+#pragma unroll
+    for (int p = 0; p < NPT; ++p) {
+        const int mm = r + p * R;
+        valid[p] = active && mm < mc;
+        vn[p] = c_v[m0 + (mm < mc ? mm : 0)];
+        Fprev[p] = 0.0;
+    }
+    const unsigned char *ring_b = reinterpret_cast<const unsigned char *>(ring) + qb0;
+    const unsigned char *stages_b = reinterpret_cast<const unsigned char *>(stages);
+    const int kb = k * 8;
+    {   // prologue: the two oldest rows of each thread's x-window go to registers
+        mbar_wait(&bars[0], 0); mbar_wait(&bars[1], 0); mbar_wait(&bars[2], 0);
+        const unsigned char *ra = ring_b + (posx ? 0 : 1) * QBB, *rb = ra + QBB;
+#pragma unroll
+        for (int p = 0; p < NPT; ++p) { fm[p] = ldsd(ra, QOFF(p)); fc[p] = ldsd(rb, QOFF(p)); }
+    }
+    __syncthreads();                                                 // rows c0-2, c0-1 consumed
+    // wall flags of the two y-faces (CTA-uniform)
+    const bool wl2 = beyond_wall_y(j - 2), wl1 = beyond_wall_y(j - 1), wu1 = beyond_wall_y(j + 1), wu2 = beyond_wall_y(j + 2);
+    const bool anyy = wl2 || wl1 || wu1 || wu2;
+    const unsigned char *gwy0 = reinterpret_cast<const unsigned char *>(A.wallg + 2 * NPAD + qa) + qb0;
+    const unsigned char *gwy1 = reinterpret_cast<const unsigned char *>(A.wallg + 3 * NPAD + qa) + qb0;
+    const unsigned char *gwx = reinterpret_cast<const unsigned char *>(A.wallg + (posx ? 0 : 1) * NPAD + qa) + qb0;
+    const int sh = posx ? 0 : 1;
+    unsigned char *out_row = reinterpret_cast<unsigned char *>(A.fnew + (size_t)j * GI * NPAD + qa) + qb0;
+
+    int xslot_new = sh;                                              // ring slot of row a + sh  (a = c0: index c0 + sh - rows_first = 2 + sh)
+    xslot_new = (2 + sh) % NSX;
+    int xw_slot = 0, xw_phase = 1;                                   // barrier slot / phase of row a+1 (index a+1-rows_first = 3 at a = c0)
+    int stage_i = 0, stage_phase = 0;
+    for (int a = c0; a <= c1; ++a) {                                 // x-face a, then cell a-1
+        const unsigned char *S = stages_b + stage_i * (L::size * 8);
+        mbar_wait(&bars[NSX + stage_i], stage_phase);
+        if (stage_i) stage_phase ^= 1;
+        stage_i ^= 1;
+        mbar_wait(&bars[xw_slot], xw_phase);                         // row a+1
+        if (++xw_slot == NSX) { xw_slot = 0; xw_phase ^= 1; }
+        const bool have_cell = a > c0;
+        // ---- x-face a: polynomial column of this thread (n = u_k; cubic in t = v_m)
+        const double *xr = reinterpret_cast<const double *>(S + L::xrec * 8);
+        const double *xlr = xr + (posx ? FR_L : FR_R);
+        const double Ek = uk * ldsd(S + (L::xrec + FR_NCOEF) * 8, kb);
+        const double p0 = Ek * fma(uk, fma(uk, fma(uk, xlr[LR_C30], xlr[LR_C20]), xlr[LR_C10]), xr[FR_C00]);
+        const double p1 = Ek * fma(uk, fma(uk, xr[FR_C21], xlr[LR_C11]), xr[FR_C01]);
+        const double p2 = Ek * fma(uk, xlr[LR_C12], xr[FR_C02]);
+        const double p3 = Ek * xr[FR_C03];
+        const double c4 = uk * xr[FR_MT4];
+        const double c45 = uk * fma(uk, xr[FR_MT5], sgx * xr[FR_MT4]);
+        const unsigned char *xm = S + L::xm * 8 + mb0;
+        const unsigned char *rn = ring_b + xslot_new * QBB;
+        if (++xslot_new == NSX) xslot_new = 0;
+        bool xw0 = false, xw1 = false, xw2 = false, xw3 = false;
+        if (a < 2 || a + 2 > GI) { xw0 = beyond_wall_x(a - 2); xw1 = beyond_wall_x(a - 1); xw2 = beyond_wall_x(a); xw3 = beyond_wall_x(a + 1); }
+        const bool anyx = xw0 || xw1 || xw2 || xw3;
+        // ---- y-faces of cell a-1: polynomial columns (t = u_k; cubic in n = v_m), L (n > 0) / R (n < 0) variants
+        const double *ylr = reinterpret_cast<const double *>(S + L::ylrec * 8), *yur = reinterpret_cast<const double *>(S + L::yurec * 8);
+        double ql0 = 0, ql1 = 0, ql2 = 0, ql3 = 0, qu0 = 0, qu1 = 0, qu2 = 0, qu3 = 0;
+        double ql1n = 0, ql2n = 0, ql3n = 0, qu1n = 0, qu2n = 0, qu3n = 0;         // R variants (mixed chunks only)
+        double gnu = 0, gpu = 0, KF = 0, KD = 0, l4 = 0, l5 = 0, u4 = 0, u5 = 0;
+        if (have_cell) {
+            auto ycol = [&](const double *yr, const double *lr, double E, double &q0_, double &q1_, double &q2_, double &q3_, bool first) {
+                if (first) q0_ = E * fma(uk, fma(uk, fma(uk, yr[FR_C03], yr[FR_C02]), yr[FR_C01]), yr[FR_C00]);
+                q1_ = E * fma(uk, fma(uk, lr[LR_C12], lr[LR_C11]), lr[LR_C10]);
+                q2_ = E * fma(uk, yr[FR_C21], lr[LR_C20]);
+                q3_ = E * lr[LR_C30];
+            };
+            const double El = ldsd(S + (L::ylrec + FR_NCOEF) * 8, kb), Eu = ldsd(S + (L::yurec + FR_NCOEF) * 8, kb);
+            ycol(ylr, ylr + (SGN >= 0 ? FR_L : FR_R), El, ql0, ql1, ql2, ql3, true);
+            ycol(yur, yur + (SGN >= 0 ? FR_L : FR_R), Eu, qu0, qu1, qu2, qu3, true);
+            if (SGN == 0) {
+                double dummy;
+                ycol(ylr, ylr + FR_R, El, dummy, ql1n, ql2n, ql3n, false);
+                ycol(yur, yur + FR_R, Eu, dummy, qu1n, qu2n, qu3n, false);
+            }
+            const double *cr = reinterpret_cast<const double *>(S + L::crec * 8);
+            gnu = ldsd(S + (L::crec + CR_NCOEF) * 8, kb); gpu = ldsd(S + (L::crec + CR_NCOEF + NUP) * 8, kb);
+            KF = cr[CR_KF]; KD = cr[CR_KD];
+            l4 = ylr[FR_MT4]; l5 = ylr[FR_MT5]; u4 = yur[FR_MT4]; u5 = yur[FR_MT5];
+        }
+        const unsigned char *y0 = S + L::yrow * 8 + qb0, *y1 = y0 + QBB, *y2 = y1 + QBB, *y3 = y2 + QBB;
+        const unsigned char *ylm = S + L::ylm * 8 + mb0, *yum = S + L::yum * 8 + mb0, *cgn = S + L::cgn * 8 + mb0, *cgp = S + L::cgp * 8 + mb0;
+        unsigned char *out = out_row + (size_t)max(a - 1, 0) * (NPAD * 8);
+
+        auto body = [&](auto fl) {                                   // fl: some stencil of this step touches a wall
+            constexpr bool FL = decltype(fl)::value;
+            // wall flags of this thread's x-window (cells a-2+sh, a-1+sh, a+sh)
+            const bool xmm = FL && (sh ? xw1 : xw0), xmc = FL && (sh ? xw2 : xw1), xmp = FL && (sh ? xw3 : xw2);
+            const double rwx = FL ? xr[FR_RHOW] : 0.0;
+#pragma unroll
+            for (int p = 0; p < NPT; ++p) {
+                const double fn = ldsd(rn, QOFF(p)), t = vn[p];
+                // x-face a (upwind cell = middle of the window)
+                double dmx = fc[p] - fm[p], dpx = fn - fc[p], fup = fc[p];
+                if (FL) { if (xmm) dmx = dpx; if (xmp) dpx = dmx; }
+                double hs = vl_half(dmx, dpx);
+                if (FL && xmc) { fup = rwx * ldsd(gwx, QOFF(p)); hs = 0.0; }
+                const double X = fma(t, fma(t, fma(t, p3, p2), p1), p0) * ldsd(xm, MOFF(p));
+                const double F = fma(c4, fup, fma(c45, hs, X));
+                const double Dx = Fprev[p] - F;
+                Fprev[p] = F;
+                const double own = posx ? fc[p] : fm[p];             // row of cell a-1
+                fm[p] = fc[p]; fc[p] = fn;
+                if (!have_cell) continue;
+                // y-faces of cell a-1: G = F / n
+                const double n = t;
+                const bool pos = SGN > 0 || (SGN == 0 && n > 0.0);
+                const double sg = pos ? 1.0 : -1.0;
+                double r0, r1, r2;                                   // the three neighbour rows of this point's stencil
+                if (SGN != 0 || pos) { r0 = ldsd(y0, QOFF(p)); r1 = ldsd(y1, QOFF(p)); r2 = ldsd(y2, QOFF(p)); }
+                else { r0 = ldsd(y1, QOFF(p)); r1 = ldsd(y2, QOFF(p)); r2 = ldsd(y3, QOFF(p)); }
+                double d1, d2, d3, ful, fuu;
+                if (pos) { d1 = r1 - r0; d2 = own - r1; d3 = r2 - own; ful = r1; fuu = own; }     // rows j-2, j-1 | j+1
+                else { d1 = own - r0; d2 = r1 - own; d3 = r2 - r1; ful = own; fuu = r1; }         // rows j-1 | j+1, j+2
+                double dl1 = d1, dl2 = d2, du2 = d2, du3 = d3;
+                if (FL) {                                            // AMB-13: one-sided slope next to a wall
+                    if (pos) { if (wl2) dl1 = dl2; if (wl1) du2 = du3; if (wu1) du3 = du2; }      // lower: (j-2, j-1, j); upper: (j-1, j, j+1)
+                    else { if (wl1) dl1 = dl2; if (wu1) dl2 = dl1; if (wu2) du3 = du2; }          // lower: (j-1, j, j+1); upper: (j, j+1, j+2)
+                }
+                double hl = vl_half(dl1, dl2), hu = vl_half(du2, du3);
+                if (FL) {
+                    if (pos && wl1) { ful = ylr[FR_RHOW] * ldsd(gwy0, QOFF(p)); hl = 0.0; }     // lower face is the ymin wall
+                    if (!pos && wu1) { fuu = yur[FR_RHOW] * ldsd(gwy1, QOFF(p)); hu = 0.0; }    // upper face is the ymax wall
+                }
+                const bool useR = SGN == 0 && !pos;
+                const double a1 = useR ? ql1n : ql1, a2 = useR ? ql2n : ql2, a3 = useR ? ql3n : ql3;
+                const double b1 = useR ? qu1n : qu1, b2 = useR ? qu2n : qu2, b3 = useR ? qu3n : qu3;
+                const double Xl = fma(n, fma(n, fma(n, a3, a2), a1), ql0) * ldsd(ylm, MOFF(p));
+                const double Xu = fma(n, fma(n, fma(n, b3, b2), b1), qu0) * ldsd(yum, MOFF(p));
+                const double Gl = fma(l4, ful, fma(fma(l5, n, sg * l4), hl, Xl));
+                const double Gu = fma(u4, fuu, fma(fma(u5, n, sg * u4), hu, Xu));
+                const double Dq = fma(n, Gl - Gu, Dx);
+                const double g = fma(ldsd(cgp, MOFF(p)), gpu, ldsd(cgn, MOFF(p)) * gnu);
+                const double fnw = fma(KF, own, fma(KD, Dq, g));     // P:L41 Eq. (3), solved for f^{n+1}
+                if (valid[p]) *reinterpret_cast<double *>(out + p * QSTEP) = fnw;
+            }
+        };
+        if (anyx || (anyy && have_cell)) body(true_c{}); else body(false_c{});
+        __syncthreads();                                             // row a and stage a are consumed
+    }
+}
+
+static_assert(StageL<3>::BYTES == G_SMEM_UPD3 && StageL<4>::BYTES == G_SMEM_UPD4, "host mirror of the shared-memory layout (ugks_jit.cu) disagrees");
+
+// one launch covers the chunk range [chunk0, chunk0 + nch): the CTA dispatches on the sign class of its chunk (the two uniform
+// classes of a cell read its records while they are in the L2)
+extern "C" __global__ void __launch_bounds__(BT + 32, G_MINB_UPD) k_flux_update(const KArgs A, const int chunk0)
+{
+    int b = blockIdx.x;
+    const int j = b % GJ; b /= GJ;
+    const int s = b % NSTRIP, c = b / NSTRIP;                        // launch order: rows fastest, then strips, then chunks
+    const int4 ch = c_chunks[chunk0 + c];
+    if (ch.z > 0) flux_update_body<1>(A, ch, j, s);
+    else if (ch.z < 0) flux_update_body<-1>(A, ch, j, s);
+#if G_NMIX > 0
+    else flux_update_body<0>(A, ch, j, s);
+#endif
+}

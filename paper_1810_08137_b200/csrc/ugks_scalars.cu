@@ -374,6 +374,26 @@ __global__ void __launch_bounds__(256) k_moments_of_f(const UgksParams P, const 
     if (lane == 0) { double *o = Wf + (size_t)c * 4; o[0] = s0; o[1] = s1; o[2] = s2; o[3] = s3; }
 }
 
+// Test aid (option "poison"): fill the shared memory of every SM with NaNs, so that a kernel of the step that reads shared
+// memory it has not written (a ragged tail, a point outside its chunk) turns into a deterministic parity failure instead of
+// depending on what the previous kernel left behind.
+__global__ void __launch_bounds__(256) k_poison_smem(int ndoubles)
+{
+    extern __shared__ double poison[];
+    for (int i = threadIdx.x; i < ndoubles; i += blockDim.x) poison[i] = __longlong_as_double(0x7ff8dead0000beefLL);
+    __syncthreads();
+    if (poison[(threadIdx.x * 37) % ndoubles] == 0.0) poison[0] = 1.0;   // keep the stores alive
+}
+int launch_poison_smem(cudaStream_t st)
+{
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+    const int bytes = 227 * 1024;
+    if (cudaFuncSetAttribute(k_poison_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) return 0;
+    k_poison_smem<<<sms, 256, bytes, st>>>(bytes / 8);
+    return 1;
+}
+
 int launch_face_scalars(const UgksParams &P, int cur, cudaStream_t st)
 {
     const int n = nfaces_x(P) + nfaces_y(P);

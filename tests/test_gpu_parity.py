@@ -20,7 +20,7 @@ TOL_1 = 1e-12
 TOL_100 = 1e-10
 
 
-def _run_pair(p, steps, W=None, f=None, threads=8):
+def _run_pair(p, steps, W=None, f=None, threads=8, options=()):
     from oracle import Oracle
     from paper_1810_08137_b200 import Ugks
     if W is None:
@@ -28,6 +28,8 @@ def _run_pair(p, steps, W=None, f=None, threads=8):
     o = Oracle(p, threads=threads)
     o.set_state(W, f)
     g = Ugks(p)
+    for name, value in options:
+        g.set_option(name, value)
     assert abs(g.dt - o.dt) <= 1e-16 * o.dt and abs(g.mu_ref - o.mu_ref) <= 1e-16 * o.mu_ref
     g.set_state(W, f)
     o.step(steps)
@@ -68,6 +70,15 @@ def test_C2_channel_reduced_100_steps():
 def test_config_velocity_grids_one_step(name, I, J):
     """Each config's velocity grid (28x28, 40x40 two chunks, 200x200 fifty chunks) on a small ragged mesh."""
     _check(_run_pair(workloads.channel_config(name, I=I, J=J), 1), TOL_1)
+
+
+@pytest.mark.parametrize("name,I,J,nuv", [("C3", 40, 12, None), ("C2", 37, 9, 49), ("C2", 36, 5, 69), ("C2", 33, 4, 29), ("C5", 6, 5, None),
+                                          ("C4", 35, 3, None), ("C1", 34, 7, 11)])
+def test_stale_shared_memory_is_never_read(name, I, J, nuv):
+    """Option "poison" NaN-fills the shared memory of every SM before each f-sized kernel: a point outside its chunk (R*NPT > MC,
+    ragged chunks of 49x49 / 69x69 grids, the one-row v = 0 chunk) or a ragged strip that read shared memory the CTA has not
+    written would poison the sums.  Three steps, so that both parities of every double buffer are used."""
+    _check(_run_pair(workloads.channel_config(name, I=I, J=J, Nuv=nuv), 3, options=(("poison", 1),)), 3 * TOL_1)
 
 
 @pytest.mark.parametrize("nu,nv", [(29, 29), (13, 9), (7, 33), (16, 12)])

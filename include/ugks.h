@@ -93,11 +93,14 @@ double ugks_mu_ref(const ugks_ctx *);
 long ugks_step_count(const ugks_ctx *);
 /* Kernels launched by this context since ugks_init (for bench.py's gpu_launches). */
 long ugks_launch_count(const ugks_ctx *);
-/* Tuning knobs (those that change the launch geometry re-compile the kernels): name in {"strip" (cells per CTA march),
- * "chunk_m" (at most that many velocity rows per chunk; may only coarsen the default chunking), "R"
- * (velocity rows processed in parallel by a CTA), "profile" (1: time every kernel of ugks_step with CUDA events),
- * "graph" (replay pairs of steps from a CUDA graph: -1 auto = on for launch-bound meshes below 4e6 points, 0 off, 1 on),
- * "poison" (test aid: 1 = NaN-fill the shared memory of every SM before each of the two f-sized kernels)}.
+/* Tuning knobs.  The two kernels that sweep f (k_cell_moments, k_flux_update) each have a launch geometry: the velocity rows
+ * are split into chunks of at most `chunk` rows (one CTA marches a strip of `strip` cells for one chunk), R rows of a chunk
+ * are processed in parallel and a thread owns ceil(chunk / R) <= 16 points.  "strip", "chunk_m" (alias "chunk"), "R" set both
+ * kernels; with the suffix "_u" (e.g. "R_u", "chunk_u") only k_flux_update, with "_m" ("R_m", "strip_m") only k_cell_moments.
+ * The chunking of k_cell_moments may only coarsen its default (the moment buffer is sized for it).  Each change re-compiles
+ * the kernel it touches.  Others: "profile" (1: time every kernel of ugks_step with CUDA events), "graph" (replay pairs of
+ * steps from a CUDA graph: -1 auto = on for launch-bound meshes, 0 off, 1 on), "poison" (test aid: 1 = NaN-fill the shared
+ * memory of every SM before each of the two f-sized kernels).
  * UGKS_EINVAL for unknown names or values that do not fit shared memory / the allocated buffers. */
 int ugks_set_option(ugks_ctx *, const char *name, int value);
 /* With option "profile" on: accumulated device time in ms and launch counts of the five kernels of a step since

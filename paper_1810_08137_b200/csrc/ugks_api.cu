@@ -10,7 +10,8 @@
 
 struct ugks_ctx {
     UgksParams P;
-    JitModule *jm;            // run-time specialised k_cell_moments / k_flux_update of this geometry (ugks_jit.cu)
+    KGeom *gm, *gu;           // launch geometries of k_cell_moments / k_flux_update (P.nchunk, P.R, ... mirror gm)
+    JitKernel *km, *ku;       // the run-time specialised kernels of these geometries (ugks_jit.cu)
     int device;               // the device the context was created on; every entry point runs there
     cudaStream_t st;
     int cur;                  // which of f[2] / W[2] holds the current state
@@ -67,74 +68,65 @@ static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 // is uniform over a CTA), each run into equal chunks of at most `cm_target` rows; rows with v = 0 and, if the node order makes
 // too many runs, everything, go to "mixed" chunks that select the side per point.  Order: [v < 0][v > 0][mixed].
 constexpr int MAXCHUNK = 4096;
-struct Chunking { int n, nneg, npos, nmix, cmax; int4 c[MAXCHUNK]; };
-struct ChunkingBox {             // heap-owned scratch (the table is 64 KB): no static buffers, the ABI is re-entrant
-    Chunking *p;
-    ChunkingBox() : p((Chunking *)calloc(1, sizeof(Chunking))) {}
-    ~ChunkingBox() { free(p); }
-    ChunkingBox(const ChunkingBox &) = delete;
-    ChunkingBox &operator=(const ChunkingBox &) = delete;
-};
 
-static void make_chunks(const double *v, int Nv, int Nu, int cm_target, Chunking *C)
+static void make_chunks(const double *v, int Nv, int Nu, int cm_target, KGeom *G)
 {
     if (cm_target < 1) cm_target = 1;
     if ((Nu & 1) && (cm_target & 1) && cm_target > 1) cm_target -= 1;
-    int4 *tmp = (int4 *)malloc(sizeof(int4) * MAXCHUNK);
-    if (!tmp) { C->n = 0; C->cmax = 0; C->nneg = C->npos = C->nmix = 0; return; }
-    int nt = 0, nruns = 0;
+    std::vector<int4> tmp;
+    int nruns = 0;
     bool fallback = false;
     for (int m = 0; m < Nv && !fallback;) {
         const int sg = v[m] > 0.0 ? 1 : (v[m] < 0.0 ? -1 : 0);
         int e = m + 1;
         while (e < Nv && (v[e] > 0.0 ? 1 : (v[e] < 0.0 ? -1 : 0)) == sg) ++e;
         const int len = e - m, parts = (len + cm_target - 1) / cm_target, rows = (len + parts - 1) / parts;
-        for (int p0 = m; p0 < e; p0 += rows) {
-            if (nt >= MAXCHUNK) { fallback = true; break; }
-            tmp[nt++] = make_int4(p0, (p0 + rows <= e ? rows : e - p0), sg, 0);
-        }
+        for (int p0 = m; p0 < e; p0 += rows) tmp.push_back(make_int4(p0, (p0 + rows <= e ? rows : e - p0), sg, 0));
         m = e;
         if (++nruns > 8) fallback = true;                            // unsorted nodes: do not shred the grid
     }
     if (fallback) {
-        nt = 0;
-        for (int m = 0; m < Nv && nt < MAXCHUNK; m += cm_target) tmp[nt++] = make_int4(m, (m + cm_target <= Nv ? cm_target : Nv - m), 0, 0);
+        tmp.clear();
+        for (int m = 0; m < Nv; m += cm_target) tmp.push_back(make_int4(m, (m + cm_target <= Nv ? cm_target : Nv - m), 0, 0));
     }
-    C->n = 0; C->cmax = 0;
+    G->chunks.clear(); G->cmax = 0;
     const int order[3] = { -1, 1, 0 };
     int cnt[3] = { 0, 0, 0 };
     for (int o = 0; o < 3; ++o)
-        for (int i = 0; i < nt; ++i)
-            if (tmp[i].z == order[o]) { C->c[C->n++] = tmp[i]; cnt[o]++; if (tmp[i].y > C->cmax) C->cmax = tmp[i].y; }
-    C->nneg = cnt[0]; C->npos = cnt[1]; C->nmix = cnt[2];
-    free(tmp);
+        for (const int4 &t : tmp)
+            if (t.z == order[o]) { G->chunks.push_back(t); cnt[o]++; if (t.y > G->cmax) G->cmax = t.y; }
+    G->nneg = cnt[0]; G->npos = cnt[1]; G->nmix = cnt[2];
 }
 
-// R rows in parallel (threads = Nu*R rounded up to a warp multiple), NPT = ceil(cmax / R) <= 7 points per thread:
-// maximise lane use x point-slot use; ties go to the larger NPT (per-face per-thread setup is amortised over NPT points)
-static void choose_R(int Nu, int cmax, int *R, int *npt)
+// R rows in parallel (threads = Nu*R rounded up to a warp multiple), NPT = ceil(cmax / R) <= 16 points per thread: maximise
+// lane use x point-slot use x a measured preference for the points per thread (the per-cell fixed work of a thread -- the
+// reduction stages of k_cell_moments, the flux-column set-up of k_flux_update -- is amortised over NPT points, registers
+// grow with NPT): k_cell_moments runs best at 7..8 (C3: R = 2, C4: R = 3), k_flux_update at 5..7 (C3: R = 2, C4: R = 4).
+static void choose_R(int kind, int Nu, int cmax, int *R, int *npt)
 {
     int best = 1; double bestscore = -1.0;
     for (int r = 1; r <= cmax && Nu * r <= 256; ++r) {
         const int n = (cmax + r - 1) / r;
-        if (n > 7) continue;
+        if (n > 16) continue;
         const int T = (Nu * r + 31) / 32 * 32;
-        // measured (C3, C4): 5 points per thread at 3 CTAs of 4-5 warps beat 7 points at 4 CTAs of 2 warps by ~3 %
-        const double score = ((double)Nu * r / T) * ((double)cmax / (r * n)) * ((n == 4 || n == 5) ? 1.08 : (n < 4 ? 0.9 : 1.0));
+        double pref;
+        if (kind == JIT_MOMENTS) pref = n >= 6 && n <= 8 ? 1.0 : (n > 8 ? 0.97 : (n == 5 ? 0.8 : 0.7));
+        else pref = n >= 5 && n <= 7 ? 1.0 : (n > 7 ? 0.9 : (n == 4 ? 0.9 : 0.75));
+        const double score = ((double)Nu * r / T) * ((double)cmax / (r * n)) * pref;
         if (score > bestscore + 1e-9) { bestscore = score; best = r; }
     }
     *R = best; *npt = (cmax + best - 1) / best;
 }
 
-static void choose_geometry(const double *v, int I, int J, int Nu, int Nv, Chunking *C, int *R, int *npt, int *strip)
+static void choose_geometry(int kind, const double *v, int I, int J, int Nu, int Nv, KGeom *G)
 {
     int cm = 800 / Nu; if (cm < 1) cm = 1; if (cm > 56) cm = 56;
-    if (Nu > 128 && cm < 7) cm = 7;                                  // wide rows: one thread per column, 7 points per thread
-    make_chunks(v, Nv, Nu, cm, C);
-    choose_R(Nu, C->cmax, R, npt);
+    if (Nu > 128) cm = kind == JIT_MOMENTS ? 14 : 10;                // wide rows: one thread per column (measured, C5)
+    make_chunks(v, Nv, Nu, cm, G);
+    choose_R(kind, Nu, G->cmax, &G->R, &G->npt);
     int s = 32;
-    while (s > 4 && (long)J * ((I + s - 1) / s) * C->n < 148L * 8) s >>= 1;
-    *strip = s;
+    while (s > 4 && (long)J * ((I + s - 1) / s) * G->nchunk() < 148L * 8) s >>= 1;
+    G->strip = s;
 }
 
 struct Layout {
@@ -152,12 +144,10 @@ static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
     L->frs = FR_NCOEF + L->NuP + L->NvP; L->crs = CR_NCOEF + 2 * L->NuP + 2 * L->NvP;
     // the moment buffer holds the chunks of the default geometry (the "chunk_m" tuning option may only coarsen it)
     if (!vg->v) return 1;
-    ChunkingBox CB;
-    if (!CB.p) return 1;
-    int R, npt, strip;
-    choose_geometry(vg->v, m->I, m->J, vg->Nu, vg->Nv, CB.p, &R, &npt, &strip);
-    size_t nchunk = (size_t)CB.p->n;
-    if (nchunk < 1) return 1;
+    KGeom G;
+    choose_geometry(JIT_MOMENTS, vg->v, m->I, m->J, vg->Nu, vg->Nv, &G);
+    size_t nchunk = (size_t)G.nchunk();
+    if (nchunk < 1 || nchunk > MAXCHUNK) return 1;
     L->nchunk_alloc = (int)nchunk;
     L->Npad = (int)Npad;
     L->resblocks = (int)((cells + 127) / 128);
@@ -181,11 +171,10 @@ static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
     return 0;
 }
 
-// chunking + (R, npt) + the column ranges by sign of u -> the geometry fields of T; returns a message on failure
-static const char *set_geometry(UgksParams &T, const Chunking *C, int R, int npt, const double *uhost)
+// the column ranges by sign of u (sorted nodes): a compile-time constant of k_cell_moments' stage 3
+static void set_u_ranges(UgksParams &T, const double *uhost)
 {
-    T.nchunk = C->n; T.nneg = C->nneg; T.npos = C->npos; T.nmix = C->nmix; T.cmax = C->cmax; T.R = R; T.npt = npt;
-    bool sorted = true;                                              // columns by sign of u (sorted nodes)
+    bool sorted = true;
     for (int k = 1; k < T.Nu; ++k) if (uhost[k] < uhost[k - 1]) sorted = false;
     T.kxm_end = T.Nu; T.kxp_begin = 0;
     if (sorted) {
@@ -195,27 +184,36 @@ static const char *set_geometry(UgksParams &T, const Chunking *C, int R, int npt
         T.kxp_begin = k0; T.kxm_end = k1;
     }
     T.s3_nsx = T.s3_nsy = 0;                                         // (the stage-3 split is a compile-time constant of the kernel)
-    if (npt < 1 || npt > 7 || R < 1 || T.Nu * R > 256 || R * npt < C->cmax) return "R / points per thread out of range";
-    if (jit_smem_flux_update(T) > 227 * 1024 || jit_smem_cell_moments(T) > 227 * 1024) return "chunk does not fit in shared memory";
+}
+// is G a launchable geometry of kernel `kind`?  returns a message if not
+static const char *check_geometry(int kind, const UgksParams &T, const KGeom &G)
+{
+    if (G.nchunk() < 1 || G.nchunk() > MAXCHUNK) return "bad chunk count";
+    if (G.npt < 1 || G.npt > 16 || G.R < 1 || T.Nu * G.R > 256 || G.R * G.npt < G.cmax) return "R / points per thread out of range";
+    if (G.strip < 1 || G.strip > 4096) return "strip out of range";
+    if (jit_smem(kind, T, G) > 227 * 1024) return "chunk does not fit in shared memory";
     return nullptr;
 }
 
-// install a chunking + (R, npt) in the context: checks buffers and shared memory, compiles / fetches the kernels of this
-// geometry, uploads the chunk table
-static int apply_geometry(ugks_ctx *c, const Chunking *C, int R, int npt, int nchunk_alloc)
+// install a launch geometry of one kernel in the context: checks buffers and shared memory, compiles / fetches the kernel of
+// this geometry; for k_cell_moments also uploads the chunk table (k_face_scalars sums the moment sets over its chunks)
+static int apply_geometry(ugks_ctx *c, int kind, const KGeom &G)
 {
     UgksParams T = c->P;
-    if (C->n > nchunk_alloc) return fail(c, UGKS_EINVAL, "%s", "too many chunks for the allocated moment buffer");
-    if (const char *why = set_geometry(T, C, R, npt, c->uhost)) return fail(c, UGKS_EINVAL, "%s", why);
+    if (kind == JIT_MOMENTS && G.nchunk() > c->nchunk_alloc) return fail(c, UGKS_EINVAL, "%s", "too many chunks for the allocated moment buffer");
+    if (const char *why = check_geometry(kind, T, G)) return fail(c, UGKS_EINVAL, "%s", why);
     CK(cudaStreamSynchronize(c->st), "apply_geometry");
     if (c->gst) cudaStreamSynchronize(c->gst);
     drop_graph(c);
-    JitModule *jm = nullptr;
+    JitKernel *jk = nullptr;
     char msg[240];
-    if (jit_get(T, C->c, c->uhost, c->wuhost, c->vhost, c->wvhost, &jm, msg, sizeof msg)) return fail(c, UGKS_ECUDA, "%s", msg);
-    CK(cudaMemcpy(c->chunks_dev, C->c, sizeof(int4) * C->n, cudaMemcpyHostToDevice), "apply_geometry");
-    c->P = T;
-    c->jm = jm;
+    if (jit_get(kind, T, G, c->uhost, c->wuhost, c->vhost, c->wvhost, &jk, msg, sizeof msg)) return fail(c, UGKS_ECUDA, "%s", msg);
+    if (kind == JIT_MOMENTS) {
+        CK(cudaMemcpy(c->chunks_dev, G.chunks.data(), sizeof(int4) * G.nchunk(), cudaMemcpyHostToDevice), "apply_geometry");
+        T.nchunk = G.nchunk(); T.nneg = G.nneg; T.npos = G.npos; T.nmix = G.nmix; T.cmax = G.cmax; T.R = G.R; T.npt = G.npt; T.strip = G.strip;
+        c->P = T;
+        *c->gm = G; c->km = jk;
+    } else { *c->gu = G; c->ku = jk; }
     return UGKS_OK;
 }
 
@@ -235,16 +233,19 @@ int ugks_jit_check(const ugks_mesh *m, const ugks_vgrid *vg, const ugks_bcs *bcs
     T.NuP = L.NuP; T.NvP = L.NvP; T.frs = L.frs; T.crs = L.crs;
     const ugks_bc *b[4] = { &bcs->xmin, &bcs->xmax, &bcs->ymin, &bcs->ymax };
     for (int s = 0; s < 4; ++s) T.bc[s] = b[s]->type;
-    ChunkingBox CB;
-    if (!CB.p) return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed");
-    int R, npt;
-    choose_geometry(vg->v, T.I, T.J, T.Nu, T.Nv, CB.p, &R, &npt, &T.strip);
-    if (const char *why = set_geometry(T, CB.p, R, npt, vg->u)) return fail(nullptr, UGKS_EINVAL, "%s", why);
-    std::vector<char> cubin;
-    std::string out;
-    const int rc = jit_compile(jit_prelude(T, CB.p->c, vg->u, vg->wu, vg->v, vg->wv), &cubin, &out, true);
-    if (log && log_bytes) snprintf(log, log_bytes, "%s", out.c_str());
-    if (rc) return fail(nullptr, UGKS_ECUDA, "JIT compile failed: %.200s", out.c_str());
+    set_u_ranges(T, vg->u);
+    std::string all;
+    for (int kind = 0; kind < 2; ++kind) {
+        KGeom G;
+        choose_geometry(kind, vg->v, T.I, T.J, T.Nu, T.Nv, &G);
+        if (const char *why = check_geometry(kind, T, G)) return fail(nullptr, UGKS_EINVAL, "%s", why);
+        std::vector<char> cubin;
+        std::string out;
+        const int rc = jit_compile(kind, jit_prelude(kind, T, G, vg->u, vg->wu, vg->v, vg->wv), &cubin, &out, true);
+        all += out;
+        if (log && log_bytes) snprintf(log, log_bytes, "%s", all.c_str());
+        if (rc) return fail(nullptr, UGKS_ECUDA, "JIT compile failed: %.200s", out.c_str());
+    }
     return UGKS_OK;
 }
 
@@ -324,11 +325,11 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     c->cells = (size_t)m->I * m->J;
     c->st = (cudaStream_t)cuda_stream;
     c->graph_mode = -1;
-    ChunkingBox CB;
-    if (!CB.p) { free(c->vhost); free(c); return fail(nullptr, UGKS_ENOMEM, "%s", "host allocation failed"); }
-    int R0, npt0;
-    choose_geometry(vg->v, P.I, P.J, P.Nu, P.Nv, CB.p, &R0, &npt0, &P.strip);
-    if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); free(c->vhost); free(c); return fail(nullptr, UGKS_ECUDA, "%s", "cudaGetDevice failed"); }
+    set_u_ranges(P, c->uhost);
+    c->gm = new KGeom(); c->gu = new KGeom();
+    KGeom G0[2];
+    for (int kind = 0; kind < 2; ++kind) choose_geometry(kind, vg->v, P.I, P.J, P.Nu, P.Nv, &G0[kind]);
+    if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c->gm; delete c->gu; free(c->vhost); free(c); return fail(nullptr, UGKS_ECUDA, "%s", "cudaGetDevice failed"); }
 
     double bcprim[16];
     for (int s = 0; s < 4; ++s) { bcprim[s * 4] = b[s]->rho; bcprim[s * 4 + 1] = b[s]->U; bcprim[s * 4 + 2] = b[s]->V; bcprim[s * 4 + 3] = b[s]->T; }
@@ -346,9 +347,11 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     if (e == cudaSuccess) e = cudaMemsetAsync(P.crec, 0, c->cells * (size_t)P.crs * 8, c->st);
     if (e == cudaSuccess) { c->launches += launch_setup(P, c->bcprim_dev, c->ghost, c->wallg, c->Wb, c->wallG, c->ghostmom, c->st); e = cudaGetLastError(); }
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
-    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); free(c->vhost); free(c); return rc; }
-    { const int rc = apply_geometry(c, CB.p, R0, npt0, c->nchunk_alloc);
-      if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); free(c->vhost); free(c); return rc; } }
+    if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); delete c->gm; delete c->gu; free(c->vhost); free(c); return rc; }
+    for (int kind = 0; kind < 2; ++kind) {
+        const int rc = apply_geometry(c, kind, G0[kind]);
+        if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); delete c->gm; delete c->gu; free(c->vhost); free(c); return rc; }
+    }
     *out = c;
     return UGKS_OK;
 }
@@ -362,6 +365,8 @@ void ugks_destroy(ugks_ctx *c)
     for (int i = 0; i < c->nev; ++i) cudaEventDestroy(c->ev[i]);
     free(c->ev);
     free(c->vhost);
+    delete c->gm;
+    delete c->gu;
     free(c);
 }
 
@@ -375,36 +380,31 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
     DevGuard dg(c);
     if (!c || !name) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     UgksParams &P = c->P;
-    if (!strcmp(name, "strip")) {
-        if (value < 1 || value > 4096) return fail(c, UGKS_EINVAL, "%s", "strip out of range");
-        ChunkingBox CB;                                              // the strip length is a compile-time constant of the kernels
-        if (!CB.p) return fail(c, UGKS_ENOMEM, "%s", "host allocation failed");
-        CK(cudaStreamSynchronize(c->st), "ugks_set_option");
-        CK(cudaMemcpy(CB.p->c, c->chunks_dev, sizeof(int4) * P.nchunk, cudaMemcpyDeviceToHost), "ugks_set_option");
-        CB.p->n = P.nchunk; CB.p->nneg = P.nneg; CB.p->npos = P.npos; CB.p->nmix = P.nmix; CB.p->cmax = P.cmax;
-        const int old = P.strip;
-        P.strip = value;
-        const int rc = apply_geometry(c, CB.p, P.R, P.npt, c->nchunk_alloc);
-        if (rc) P.strip = old;
-        return rc;
-    }
-    if (!strcmp(name, "chunk_m")) {                                  // re-chunk with at most `value` rows per chunk
-        if (value < 1 || value > 56) return fail(c, UGKS_EINVAL, "%s", "chunk_m out of range");
-        ChunkingBox CB;
-        if (!CB.p) return fail(c, UGKS_ENOMEM, "%s", "host allocation failed");
-        make_chunks(c->vhost, P.Nv, P.Nu, value, CB.p);
-        int R, npt;
-        choose_R(P.Nu, CB.p->cmax, &R, &npt);
-        return apply_geometry(c, CB.p, R, npt, c->nchunk_alloc);
-    }
-    if (!strcmp(name, "R")) {
-        if (value < 1 || P.Nu * value > 256) return fail(c, UGKS_EINVAL, "%s", "R out of range");
-        ChunkingBox CB;
-        if (!CB.p) return fail(c, UGKS_ENOMEM, "%s", "host allocation failed");
-        CK(cudaStreamSynchronize(c->st), "ugks_set_option");
-        CK(cudaMemcpy(CB.p->c, c->chunks_dev, sizeof(int4) * P.nchunk, cudaMemcpyDeviceToHost), "ugks_set_option");
-        CB.p->n = P.nchunk; CB.p->nneg = P.nneg; CB.p->npos = P.npos; CB.p->nmix = P.nmix; CB.p->cmax = P.cmax;
-        return apply_geometry(c, CB.p, value, (P.cmax + value - 1) / value, c->nchunk_alloc);
+    // launch geometry of the two f-sized kernels; a "_u" suffix addresses k_flux_update alone, no suffix both kernels
+    // ("R" and "chunk_m" / "strip" re-compile the kernel they change)
+    {
+        const size_t len = strlen(name);
+        const bool only_u = len > 2 && !strcmp(name + len - 2, "_u"), only_m = len > 2 && !strcmp(name + len - 2, "_m") && strcmp(name, "chunk_m");
+        char base[32];
+        snprintf(base, sizeof base, "%.*s", (int)((only_u || only_m) ? len - 2 : len), name);
+        if (!strcmp(base, "strip") || !strcmp(base, "chunk") || !strcmp(base, "chunk_m") || !strcmp(base, "R")) {
+            for (int kind = 0; kind < 2; ++kind) {
+                if ((kind == JIT_MOMENTS && only_u) || (kind == JIT_UPDATE && only_m)) continue;
+                KGeom G = kind == JIT_MOMENTS ? *c->gm : *c->gu;
+                if (!strcmp(base, "strip")) G.strip = value;
+                else if (!strcmp(base, "R")) {
+                    if (value < 1 || P.Nu * value > 256) return fail(c, UGKS_EINVAL, "%s", "R out of range");
+                    G.R = value; G.npt = (G.cmax + value - 1) / value;
+                } else {                                             // re-chunk with at most `value` rows per chunk
+                    if (value < 1 || value > 56) return fail(c, UGKS_EINVAL, "%s", "chunk rows out of range");
+                    make_chunks(c->vhost, P.Nv, P.Nu, value, &G);
+                    choose_R(kind, P.Nu, G.cmax, &G.R, &G.npt);
+                }
+                const int rc = apply_geometry(c, kind, G);
+                if (rc) return rc;
+            }
+            return UGKS_OK;
+        }
     }
     if (!strcmp(name, "profile")) { c->profile = value != 0; return UGKS_OK; }
     if (!strcmp(name, "poison")) { c->poison = value != 0; drop_graph(c); return UGKS_OK; }
@@ -447,12 +447,12 @@ static long enqueue_step(ugks_ctx *c, int cur, cudaStream_t st)
 {
     long n = 0;
     if (c->poison) n += launch_poison_smem(st);
-    n += jit_launch_cell_moments(c->jm, c->P, cur, st);
+    n += jit_launch_cell_moments(c->km, c->P, *c->gm, cur, st);
     n += launch_face_scalars(c->P, cur, st);
     n += launch_cell_scalars(c->P, cur, c->resblocks, st);
     n += launch_tables(c->P, st);
     if (c->poison) n += launch_poison_smem(st);
-    n += jit_launch_flux_update(c->jm, c->P, cur, st);
+    n += jit_launch_flux_update(c->ku, c->P, *c->gu, cur, st);
     return n;
 }
 
@@ -514,7 +514,7 @@ int ugks_step(ugks_ctx *c, int n)
         cudaEvent_t *e = c->profile ? c->ev + c->nev_used : nullptr;
         if (c->poison) c->launches += launch_poison_smem(c->st);
         if (e) cudaEventRecord(e[0], c->st);
-        c->launches += jit_launch_cell_moments(c->jm, c->P, c->cur, c->st);       // R, S1, S7 sums (both directions)
+        c->launches += jit_launch_cell_moments(c->km, c->P, *c->gm, c->cur, c->st);       // R, S1, S7 sums (both directions)
         if (e) cudaEventRecord(e[1], c->st);
         c->launches += launch_face_scalars(c->P, c->cur, c->st);       // S2..S5, wall density
         if (e) cudaEventRecord(e[2], c->st);
@@ -523,7 +523,7 @@ int ugks_step(ugks_ctx *c, int n)
         c->launches += launch_tables(c->P, c->st);                     // S6 / U2 separable Maxwellian factors
         if (c->poison) c->launches += launch_poison_smem(c->st);
         if (e) cudaEventRecord(e[4], c->st);
-        c->launches += jit_launch_flux_update(c->jm, c->P, c->cur, c->st);        // R, S6, S8, U3
+        c->launches += jit_launch_flux_update(c->ku, c->P, *c->gu, c->cur, c->st);        // R, S6, S8, U3
         if (e) { cudaEventRecord(e[5], c->st); c->nev_used += 6; }
         c->cur ^= 1;
         c->steps += 1;

@@ -63,7 +63,7 @@ struct UgksParams {
     int nneg, npos, nmix;            // chunks per class
     int cmax;                        // rows of the largest chunk
     int R;                           // velocity rows processed in parallel by one CTA (threads = Nu*R rounded up to 32)
-    int npt;                         // velocity points per thread = ceil(cmax / R), 1..7 (template parameter)
+    int npt;                         // velocity points per thread = ceil(cmax / R), 1..16 (compile-time constant of the JIT kernels)
     int kxm_end, kxp_begin;          // columns with u_k <= 0 are [0, kxm_end), with u_k >= 0 [kxp_begin, Nu) (sorted nodes; else 0..Nu)
     int s3_nsx, s3_nsy;              // unused (the stage-3 split of k_cell_moments is a compile-time constant)
 };

@@ -23,28 +23,28 @@
 namespace {
 
 std::mutex g_mu;
-std::map<std::string, JitModule *> g_cache;
+std::map<std::string, JitKernel *> g_cache;
 
 int pad2i(int x) { return (x + 1) & ~1; }
 int cdivi(int a, int b) { return (a + b - 1) / b; }
 
 // host mirrors of MomL<MIXED>::BYTES and StageL<NY>::BYTES (the device code static_asserts that they agree)
-int smem_mom(const UgksParams &P, bool mixed)
+int smem_mom(const UgksParams &P, const KGeom &G, bool mixed)
 {
-    const int BT = (P.Nu * P.R + 31) / 32 * 32, QB = pad2i(P.cmax * P.Nu + 1);
+    const int BT = (P.Nu * G.R + 31) / 32 * 32, QB = pad2i(G.cmax * P.Nu + 1);
     const int NA = mixed ? 20 : 13, NC = mixed ? 23 : 16, ny = mixed ? 26 : 13;
     const int lenx = P.kxm_end > P.Nu - P.kxp_begin ? P.kxm_end : P.Nu - P.kxp_begin;
     int per = P.Nu;
     for (int q = 1; q <= P.Nu; ++q) if (26 * cdivi(lenx, q) + ny * cdivi(P.Nu, q) <= BT) { per = q; break; }
-    const int nitem = 26 * cdivi(lenx, per) + ny * cdivi(P.Nu, per), NUS = P.Nu | 1, NROW = P.R * P.npt + 1;
-    const int total = 3 * QB + 4 * QB + (P.R == 1 ? 0 : 2 * NA * BT) + pad2i(2 * NC * NUS) + pad2i(13 * NUS) + pad2i(NROW * 6) +
+    const int nitem = 26 * cdivi(lenx, per) + ny * cdivi(P.Nu, per), NUS = P.Nu | 1, NROW = G.R * G.npt + 1;
+    const int total = 3 * QB + 4 * QB + (G.R == 1 ? 0 : 2 * NA * BT) + pad2i(2 * NC * NUS) + pad2i(13 * NUS) + pad2i(NROW * 6) +
                       pad2i(2 * nitem) + 5;
     return total * 8;
 }
-int smem_upd(const UgksParams &P, int ny)
+int smem_upd(const UgksParams &P, const KGeom &G, int ny)
 {
-    const int QB = pad2i(P.cmax * P.Nu + 1), CMP = pad2i(P.cmax + 1);
-    const int size = ny * QB + 3 * (FR_NCOEF + P.NuP) + 3 * CMP + (CR_NCOEF + 2 * P.NuP) + 2 * CMP;
+    const int QB = pad2i(G.cmax * P.Nu + 1);
+    const int size = ny * QB + 3 * P.frs + P.crs;
     return (3 * QB + 2 * size) * 8 + 5 * 8;
 }
 // CTAs per SM for __launch_bounds__: what shared memory allows, capped so that a thread keeps at least `regs` registers
@@ -55,11 +55,15 @@ int min_blocks(int threads, int smem, int regs)
     int b = by_smem < by_regs ? by_smem : by_regs;
     return b < 1 ? 1 : (b > 16 ? 16 : b);
 }
+int threads_of(int kind, const UgksParams &P, const KGeom &G)
+{
+    return (P.Nu * G.R + 31) / 32 * 32 + (kind == JIT_MOMENTS ? 32 : 0);      // k_cell_moments: + the producer warp
+}
 
 std::string dir_of_this_library()
 {
     Dl_info info;
-    if (!dladdr((const void *)&jit_smem_cell_moments, &info) || !info.dli_fname) return ".";
+    if (!dladdr((const void *)&jit_smem, &info) || !info.dli_fname) return ".";
     std::string p(info.dli_fname);
     const size_t s = p.rfind('/');
     return s == std::string::npos ? "." : p.substr(0, s);
@@ -86,28 +90,35 @@ void add_doubles(std::string &s, const char *name, const double *a, int n)
 
 }  // namespace
 
-size_t jit_smem_cell_moments(const UgksParams &P) { return (size_t)smem_mom(P, P.nmix > 0); }
-size_t jit_smem_flux_update(const UgksParams &P) { return (size_t)smem_upd(P, P.nmix > 0 ? 4 : 3); }
-
-std::string jit_prelude(const UgksParams &P, const int4 *chunks, const double *u, const double *wu, const double *v, const double *wv)
+size_t jit_smem(int kind, const UgksParams &P, const KGeom &G)
 {
-    const int threads = (P.Nu * P.R + 31) / 32 * 32 + 32;
-    const int sm_u = smem_mom(P, false), sm_m = smem_mom(P, true), su3 = smem_upd(P, 3), su4 = smem_upd(P, 4);
+    if (kind == JIT_MOMENTS) return (size_t)smem_mom(P, G, G.nmix > 0);
+    return (size_t)smem_upd(P, G, G.nmix > 0 ? 4 : 3);
+}
+
+std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const double *u, const double *wu, const double *v, const double *wv)
+{
+    const int threads = threads_of(kind, P, G);
     std::string s;
     char b[256];
 #define DEF(name, val) do { snprintf(b, sizeof b, "#define %s %d\n", name, (int)(val)); s += b; } while (0)
     DEF("G_I", P.I); DEF("G_J", P.J); DEF("G_NU", P.Nu); DEF("G_NV", P.Nv); DEF("G_NPAD", P.Npad); DEF("G_NUP", P.NuP); DEF("G_NVP", P.NvP);
     DEF("G_FRS", P.frs); DEF("G_CRS", P.crs);
     DEF("G_BC0", P.bc[0]); DEF("G_BC1", P.bc[1]); DEF("G_BC2", P.bc[2]); DEF("G_BC3", P.bc[3]);
-    DEF("G_NCHUNK", P.nchunk); DEF("G_NMIX", P.nmix); DEF("G_MC", P.cmax); DEF("G_R", P.R); DEF("G_NPT", P.npt); DEF("G_STRIP", P.strip);
-    DEF("G_KXM_END", P.kxm_end); DEF("G_KXP_BEGIN", P.kxp_begin);
-    { int ragged = 0; for (int i = 0; i < P.nchunk; ++i) if (chunks[i].y != P.cmax) ragged = 1; DEF("G_RAGGED", ragged); }
-    DEF("G_SMEM_MOM", sm_u); DEF("G_SMEM_MOMX", sm_m); DEF("G_SMEM_UPD3", su3); DEF("G_SMEM_UPD4", su4);
-    DEF("G_MINB_MOM", min_blocks(threads, sm_u, 128)); DEF("G_MINB_MOMX", min_blocks(threads, sm_m, 128));
-    DEF("G_MINB_UPD", min_blocks(threads, P.nmix > 0 ? su4 : su3, 128));
+    DEF("G_NCHUNK", G.nchunk()); DEF("G_NMIX", G.nmix); DEF("G_MC", G.cmax); DEF("G_R", G.R); DEF("G_NPT", G.npt); DEF("G_STRIP", G.strip);
+    DEF("G_KXM_END", P.kxm_end); DEF("G_KXP_BEGIN", P.kxp_begin); DEF("G_RAGGED", G.ragged() ? 1 : 0);
+    if (kind == JIT_MOMENTS) {
+        const int sm_u = smem_mom(P, G, false), sm_m = smem_mom(P, G, true);
+        DEF("G_SMEM_MOM", sm_u); DEF("G_SMEM_MOMX", sm_m);
+        DEF("G_MINB_MOM", min_blocks(threads, sm_u, 128)); DEF("G_MINB_MOMX", min_blocks(threads, sm_m, 128));
+    } else {
+        const int su3 = smem_upd(P, G, 3), su4 = smem_upd(P, G, 4);
+        DEF("G_SMEM_UPD3", su3); DEF("G_SMEM_UPD4", su4);
+        DEF("G_MINB_UPD", min_blocks(threads, G.nmix > 0 ? su4 : su3, 128));
+    }
 #undef DEF
     s += "__constant__ int4 c_chunks[] = {";
-    for (int i = 0; i < P.nchunk; ++i) { snprintf(b, sizeof b, "%s{%d, %d, %d, 0}", i ? ", " : "", chunks[i].x, chunks[i].y, chunks[i].z); s += b; }
+    for (int i = 0; i < G.nchunk(); ++i) { snprintf(b, sizeof b, "%s{%d, %d, %d, 0}", i ? ", " : "", G.chunks[i].x, G.chunks[i].y, G.chunks[i].z); s += b; }
     s += "};\n";
     if (const char *extra = getenv("UGKS_JIT_DEFS")) { s += extra; s += "\n"; }      // developer aid: extra #define lines for experiments
     add_doubles(s, "c_u", u, P.Nu); add_doubles(s, "c_wu", wu, P.Nu); add_doubles(s, "c_v", v, P.Nv); add_doubles(s, "c_wv", wv, P.Nv);
@@ -115,24 +126,23 @@ std::string jit_prelude(const UgksParams &P, const int4 *chunks, const double *u
 }
 
 // compile (no device needed).  On success *cubin holds the image; log receives the NVRTC log (ptxas -v lines with verbose).
-int jit_compile(const std::string &prelude, std::vector<char> *cubin, std::string *log, bool verbose)
+int jit_compile(int kind, const std::string &prelude, std::vector<char> *cubin, std::string *log, bool verbose)
 {
-    static const char *names[3] = { "ugks_jit_common.cuh", "ugks_jit_moments.cuh", "ugks_jit_update.cuh" };
-    const std::string dir = dir_of_this_library() + "/csrc/";
-    std::string hdr[3];
-    for (int i = 0; i < 3; ++i)
-        if (!read_file(dir + names[i], &hdr[i])) { *log = "cannot read " + dir + names[i]; return 1; }
-    const std::string src = prelude + "#include \"ugks_jit_moments.cuh\"\n#include \"ugks_jit_update.cuh\"\n";
-    const char *hsrc[3] = { hdr[0].c_str(), hdr[1].c_str(), hdr[2].c_str() };
+    // the headers are read from disk through an include path, so that -lineinfo records their real paths (ncu --import-source)
+    const std::string dir = dir_of_this_library() + "/csrc";
+    std::string probe;
+    if (!read_file(dir + "/ugks_jit_common.cuh", &probe)) { *log = "cannot read " + dir + "/ugks_jit_common.cuh"; return 1; }
+    const std::string src = prelude + (kind == JIT_MOMENTS ? "#include \"ugks_jit_moments.cuh\"\n" : "#include \"ugks_jit_update.cuh\"\n");
     nvrtcProgram prog;
-    if (nvrtcCreateProgram(&prog, src.c_str(), (dir + "ugks_jit_generated.cu").c_str(), 3, hsrc, names) != NVRTC_SUCCESS) { *log = "nvrtcCreateProgram failed"; return 1; }
-    std::vector<const char *> opts = { "--gpu-architecture=sm_100a", "-lineinfo", "--std=c++17", "-default-device" };
+    if (nvrtcCreateProgram(&prog, src.c_str(), (dir + (kind == JIT_MOMENTS ? "/ugks_jit_generated_moments.cu" : "/ugks_jit_generated_update.cu")).c_str(), 0, nullptr, nullptr) != NVRTC_SUCCESS) { *log = "nvrtcCreateProgram failed"; return 1; }
+    const std::string inc = "--include-path=" + dir;
+    std::vector<const char *> opts = { "--gpu-architecture=sm_100a", "-lineinfo", "--std=c++17", "-default-device", inc.c_str() };
     if (verbose) opts.push_back("--ptxas-options=-v");
     const nvrtcResult rc = nvrtcCompileProgram(prog, (int)opts.size(), opts.data());
     size_t n = 0;
     nvrtcGetProgramLogSize(prog, &n);
     log->assign(n, '\0');
-    if (n) nvrtcGetProgramLog(prog, &(*log)[0]);
+    if (n) { nvrtcGetProgramLog(prog, &(*log)[0]); log->resize(strlen(log->c_str())); }
     if (rc != NVRTC_SUCCESS) { nvrtcDestroyProgram(&prog); *log = std::string("NVRTC: ") + nvrtcGetErrorString(rc) + "\n" + *log; return 1; }
     nvrtcGetCUBINSize(prog, &n);
     cubin->resize(n);
@@ -144,33 +154,33 @@ int jit_compile(const std::string &prelude, std::vector<char> *cubin, std::strin
     return n ? 0 : 1;
 }
 
-int jit_get(const UgksParams &P, const int4 *chunks, const double *u, const double *wu, const double *v, const double *wv,
-            JitModule **out, char *err, size_t errlen)
+int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, const double *wu, const double *v, const double *wv,
+            JitKernel **out, char *err, size_t errlen)
 {
-    const std::string pre = jit_prelude(P, chunks, u, wu, v, wv);
+    const std::string pre = jit_prelude(kind, P, G, u, wu, v, wv);
+    const std::string key = (kind == JIT_MOMENTS ? "M:" : "U:") + pre;
     std::lock_guard<std::mutex> lock(g_mu);
-    JitModule *m = nullptr;
-    auto it = g_cache.find(pre);
+    JitKernel *m = nullptr;
+    auto it = g_cache.find(key);
     if (it != g_cache.end()) m = it->second;
     else {
         std::vector<char> cubin;
         std::string log;
-        if (jit_compile(pre, &cubin, &log, false)) { snprintf(err, errlen, "JIT compile failed: %.200s", log.c_str()); return 1; }
-        m = new JitModule();
+        if (jit_compile(kind, pre, &cubin, &log, false)) { snprintf(err, errlen, "JIT compile failed: %.200s", log.c_str()); return 1; }
+        m = new JitKernel();
         m->image.swap(cubin);
         cudaError_t e = cudaLibraryLoadData(&m->lib, m->image.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
-        if (e == cudaSuccess) e = cudaLibraryGetKernel(&m->k_mom, m->lib, "k_cell_moments");
-        if (e == cudaSuccess) e = cudaLibraryGetKernel(&m->k_upd, m->lib, "k_flux_update");
-        if (e == cudaSuccess && P.nmix > 0) e = cudaLibraryGetKernel(&m->k_momx, m->lib, "k_cell_moments_mixed");
+        if (e == cudaSuccess) e = cudaLibraryGetKernel(&m->k, m->lib, kind == JIT_MOMENTS ? "k_cell_moments" : "k_flux_update");
+        if (e == cudaSuccess && kind == JIT_MOMENTS && G.nmix > 0) e = cudaLibraryGetKernel(&m->kx, m->lib, "k_cell_moments_mixed");
         if (e != cudaSuccess) { snprintf(err, errlen, "JIT load failed: %s", cudaGetErrorString(e)); delete m; return 1; }
-        m->threads = (P.Nu * P.R + 31) / 32 * 32 + 32;
-        m->smem_mom = smem_mom(P, false); m->smem_momx = smem_mom(P, true); m->smem_upd = smem_upd(P, P.nmix > 0 ? 4 : 3);
-        g_cache[pre] = m;
+        m->threads = threads_of(kind, P, G);
+        if (kind == JIT_MOMENTS) { m->smem = smem_mom(P, G, false); m->smemx = smem_mom(P, G, true); }
+        else m->smem = smem_upd(P, G, G.nmix > 0 ? 4 : 3);
+        g_cache[key] = m;
     }
     // shared-memory opt-in: a function attribute of the CURRENT device, set for every context (cheap, idempotent)
-    cudaError_t e = cudaFuncSetAttribute((const void *)m->k_mom, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem_mom);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)m->k_upd, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem_upd);
-    if (e == cudaSuccess && P.nmix > 0) e = cudaFuncSetAttribute((const void *)m->k_momx, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem_momx);
+    cudaError_t e = cudaFuncSetAttribute((const void *)m->k, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem);
+    if (e == cudaSuccess && m->kx) e = cudaFuncSetAttribute((const void *)m->kx, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smemx);
     if (e != cudaSuccess) { snprintf(err, errlen, "shared-memory opt-in failed: %s", cudaGetErrorString(e)); return 1; }
     *out = m;
     return 0;
@@ -184,32 +194,32 @@ static KArgs_h make_args(const UgksParams &P, int cur)
     return a;
 }
 
-int jit_launch_cell_moments(const JitModule *m, const UgksParams &P, int cur, cudaStream_t st)
+int jit_launch_cell_moments(const JitKernel *m, const UgksParams &P, const KGeom &G, int cur, cudaStream_t st)
 {
-    const int nstrip = (P.I + P.strip - 1) / P.strip;
+    const int nstrip = (P.I + G.strip - 1) / G.strip;
     KArgs_h a = make_args(P, cur);
     int n = 0;
-    if (P.nneg + P.npos) {
+    if (G.nneg + G.npos) {
         int chunk0 = 0;
         void *args[2] = { &a, &chunk0 };
-        cudaLaunchKernel((const void *)m->k_mom, dim3(P.J * nstrip * (P.nneg + P.npos)), dim3(m->threads), args, m->smem_mom, st);
+        cudaLaunchKernel((const void *)m->k, dim3(P.J * nstrip * (G.nneg + G.npos)), dim3(m->threads), args, m->smem, st);
         ++n;
     }
-    if (P.nmix) {
-        int chunk0 = P.nneg + P.npos;
+    if (G.nmix) {
+        int chunk0 = G.nneg + G.npos;
         void *args[2] = { &a, &chunk0 };
-        cudaLaunchKernel((const void *)m->k_momx, dim3(P.J * nstrip * P.nmix), dim3(m->threads), args, m->smem_momx, st);
+        cudaLaunchKernel((const void *)m->kx, dim3(P.J * nstrip * G.nmix), dim3(m->threads), args, m->smemx, st);
         ++n;
     }
     return n;
 }
 
-int jit_launch_flux_update(const JitModule *m, const UgksParams &P, int cur, cudaStream_t st)
+int jit_launch_flux_update(const JitKernel *m, const UgksParams &P, const KGeom &G, int cur, cudaStream_t st)
 {
-    const int nstrip = (P.I + P.strip - 1) / P.strip;
+    const int nstrip = (P.I + G.strip - 1) / G.strip;
     KArgs_h a = make_args(P, cur);
     int chunk0 = 0;
     void *args[2] = { &a, &chunk0 };
-    cudaLaunchKernel((const void *)m->k_upd, dim3(P.J * nstrip * P.nchunk), dim3(m->threads), args, m->smem_upd, st);
+    cudaLaunchKernel((const void *)m->k, dim3(P.J * nstrip * G.nchunk()), dim3(m->threads), args, m->smem, st);
     return 1;
 }

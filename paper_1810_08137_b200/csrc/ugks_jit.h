@@ -9,19 +9,30 @@ struct KArgs_h {                     // host mirror of KArgs (ugks_jit_common.cu
     const double *fcur; double *fnew; double *cmom; const double *frec0, *frec1, *crec, *ghost, *wallg;
 };
 
-struct JitModule {
-    std::vector<char> image;         // cubin (kept alive for the library)
-    cudaLibrary_t lib = nullptr;
-    cudaKernel_t k_mom = nullptr, k_momx = nullptr, k_upd = nullptr;
-    int threads = 0, smem_mom = 0, smem_momx = 0, smem_upd = 0;
+enum { JIT_MOMENTS = 0, JIT_UPDATE = 1 };
+
+// Launch geometry of ONE of the two f-sized kernels (each has its own: k_cell_moments likes more points per thread than
+// k_flux_update).  Velocity-row chunks are sorted [v < 0][v > 0][mixed]; (m0, mc, sign, 0) each.
+struct KGeom {
+    int nneg = 0, npos = 0, nmix = 0, cmax = 0, R = 1, npt = 1, strip = 32;
+    std::vector<int4> chunks;
+    int nchunk() const { return (int)chunks.size(); }
+    bool ragged() const { for (const int4 &c : chunks) if (c.y != cmax) return true; return false; }
 };
 
-size_t jit_smem_cell_moments(const UgksParams &P);
-size_t jit_smem_flux_update(const UgksParams &P);
-std::string jit_prelude(const UgksParams &P, const int4 *chunks, const double *u, const double *wu, const double *v, const double *wv);
-int jit_compile(const std::string &prelude, std::vector<char> *cubin, std::string *log, bool verbose);
-// module for this geometry (compiled once per process and prelude); sets the shared-memory opt-in on the current device
-int jit_get(const UgksParams &P, const int4 *chunks, const double *u, const double *wu, const double *v, const double *wv,
-            JitModule **out, char *err, size_t errlen);
-int jit_launch_cell_moments(const JitModule *m, const UgksParams &P, int cur, cudaStream_t st);
-int jit_launch_flux_update(const JitModule *m, const UgksParams &P, int cur, cudaStream_t st);
+struct JitKernel {
+    std::vector<char> image;         // cubin (kept alive for the library)
+    cudaLibrary_t lib = nullptr;
+    cudaKernel_t k = nullptr, kx = nullptr;      // the kernel; for JIT_MOMENTS also the variant for mixed-sign chunks
+    int threads = 0, smem = 0, smemx = 0;
+};
+
+// dynamic shared memory of a kernel of this geometry (the larger of its variants)
+size_t jit_smem(int kind, const UgksParams &P, const KGeom &G);
+std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const double *u, const double *wu, const double *v, const double *wv);
+int jit_compile(int kind, const std::string &prelude, std::vector<char> *cubin, std::string *log, bool verbose);
+// kernel for this geometry (compiled once per process and prelude); sets the shared-memory opt-in on the current device
+int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, const double *wu, const double *v, const double *wv,
+            JitKernel **out, char *err, size_t errlen);
+int jit_launch_cell_moments(const JitKernel *m, const UgksParams &P, const KGeom &G, int cur, cudaStream_t st);
+int jit_launch_flux_update(const JitKernel *m, const UgksParams &P, const KGeom &G, int cur, cudaStream_t st);

@@ -131,8 +131,12 @@ __device__ __forceinline__ double vl_half(double dm, double dp)
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));
     const double e = fma(-s, r, 1.0);
+#ifdef UGKS_VL_NEWTON2                                               // experiment: quadratic step, error e^2 ~ 2^-46
+    r = fma(r, e, r);
+#else
     const double t = fma(e, e, e);
     r = fma(r, t, r);
+#endif
     const double hs = pr * r;
     return __double2hiint(pr) > 0 ? hs : 0.0;
 }

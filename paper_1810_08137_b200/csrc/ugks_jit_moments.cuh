@@ -352,6 +352,10 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
 
 static_assert(MomL<false>::BYTES == G_SMEM_MOM && MomL<true>::BYTES == G_SMEM_MOMX, "host mirror of the shared-memory layout (ugks_jit.cu) disagrees");
 
+#ifdef UGKS_MINB_MOM                                                // experiment override (UGKS_JIT_DEFS)
+#undef G_MINB_MOM
+#define G_MINB_MOM UGKS_MINB_MOM
+#endif
 extern "C" __global__ void __launch_bounds__(BT + 32, G_MINB_MOM) k_cell_moments(const KArgs A, const int chunk0)
 {
     cell_moments_body<false>(A, chunk0);

@@ -12,27 +12,24 @@
 //     shared-memory ring fed by 1-D TMA bulk copies.  The x-face flux is evaluated once per face and carried in registers to
 //     the next cell.
 //   * y-stencil: three rows ((j-2, j-1, j+1) for v > 0, (j-1, j+1, j+2) for v < 0) are TMA-staged per cell, double-buffered,
-//     together with the records of the step (face and cell coefficients, separable factors).
+//     together with the records of the step (face and cell coefficients, separable factors; whole records, one copy each).
 //   * f^{n+1} is written straight from registers: f crosses HBM once each way in this kernel.
+//   * there is no producer warp: after the barrier that ends step a, one lane of warp (a mod W) issues the 8 bulk copies of
+//     step a+2 / row a+3 (with compile-time geometry that is a few dozen instructions), so every resident warp computes and
+//     no warp's registers idle.
 #pragma once
 #include "ugks_jit_common.cuh"
 
 constexpr int NSX = 3;                                               // x-ring slots: rows a, a+1 live, a+2 in flight
-constexpr int CMP = pad2c(MC + 1);                                   // doubles per staged piece of a per-row (m) table
 
 template <int NY>
 struct StageL {                                                      // offsets in doubles inside one step stage
     static constexpr int yrow = 0;
     static constexpr int xrec = yrow + NY * QB;
-    static constexpr int xm = xrec + FR_NCOEF + NUP;
-    static constexpr int ylrec = xm + CMP;
-    static constexpr int ylm = ylrec + FR_NCOEF + NUP;
-    static constexpr int yurec = ylm + CMP;
-    static constexpr int yum = yurec + FR_NCOEF + NUP;
-    static constexpr int crec = yum + CMP;
-    static constexpr int cgn = crec + CR_NCOEF + 2 * NUP;
-    static constexpr int cgp = cgn + CMP;
-    static constexpr int size = cgp + CMP;
+    static constexpr int ylrec = xrec + FRS;
+    static constexpr int yurec = ylrec + FRS;
+    static constexpr int crec = yurec + FRS;
+    static constexpr int size = crec + CRS;
     static constexpr int BYTES = (NSX * QB + 2 * size) * 8 + (NSX + 2) * 8;
 };
 
@@ -45,10 +42,8 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     const int c0 = s * STRIP, c1 = min(c0 + STRIP, GI);              // cells [c0, c1) of row j
     const int m0 = ch.x, mc = ch.y;
     const int q0 = m0 * NU, qa = q0 & ~1, qsh = q0 - qa;
-    const int ma = m0 & ~1, msh = m0 - ma;
     const uint32_t bytes = (uint32_t)(pad2c(mc * NU + qsh) * 8);
-    const uint32_t mbytes = (uint32_t)(pad2c(mc + msh) * 8);
-    constexpr uint32_t kbytes = (FR_NCOEF + NUP) * 8, cbytes = (CR_NCOEF + 2 * NUP) * 8;
+    constexpr uint32_t fbytes = FRS * 8, cbytes = CRS * 8;
 
     double *ring = reinterpret_cast<double *>(smem_raw);             // [NSX][QB]
     double *stages = ring + NSX * QB;                                // [2][L::size]
@@ -59,69 +54,46 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     const int k = active ? tid % NU : 0, r = active ? tid / NU : 0;
     const double *fcur = A.fcur;
     const int rows_first = c0 - 2, rows_last = c1 + 1;
-    if (tid >= BT) {                                                 // ---- producer warp: one lane issues every bulk copy
-        const bool lead = tid == BT;
-        // global sources of a step, linear in the cell index: y-neighbour rows, face records, cell records
-        const int djs[4] = { SGN == 0 ? -2 : (SGN > 0 ? -2 : -1), SGN == 0 ? -1 : (SGN > 0 ? -1 : 1), SGN == 0 ? 1 : (SGN > 0 ? 1 : 2), 2 };
-        const double *yb[NY];
-        int yst[NY];
-#pragma unroll
-        for (int d = 0; d < NY; ++d) yb[d] = yrow_base(fcur, A.ghost, j + djs[d], &yst[d]) + qa;
-        const double *xrp = A.frec0 + (size_t)j * (GI + 1) * FRS;
-        const double *ylp = A.frec1 + (size_t)j * GI * FRS, *yup = ylp + (size_t)GI * FRS;
-        const double *crp = A.crec + (size_t)j * GI * CRS;
-        const int moffK = FR_NCOEF + NUP + ma, moffC = CR_NCOEF + 2 * NUP + ma;
-
-        auto issue_x = [&](int row) {
-            const int sl = (row - rows_first) % NSX;
-            mbar_expect_tx(&bars[sl], bytes);
-            tma_load_1d(ring + sl * QB, xrow_ptr(fcur, A.ghost, row, j) + qa, bytes, &bars[sl]);
-        };
-        // stage of step st: record of x-face st and, for cell st-1, its y-neighbour rows, y-face records and cell record
-        auto issue_stage = [&](int st) {
-            const int sl = (st - c0) & 1;
-            double *S = stages + sl * L::size;
-            uint64_t *bar = &bars[NSX + sl];
-            const bool have_cell = st > c0;
-            mbar_expect_tx(bar, kbytes + mbytes + (have_cell ? NY * bytes + 2 * (kbytes + mbytes) + cbytes + 2 * mbytes : 0));
-            const double *xr = xrp + (size_t)st * FRS;
-            tma_load_1d(S + L::xrec, xr, kbytes, bar);
-            tma_load_1d(S + L::xm, xr + moffK, mbytes, bar);
-            if (have_cell) {
-                const size_t cell = st - 1;
-#pragma unroll
-                for (int d = 0; d < NY; ++d) tma_load_1d(S + L::yrow + d * QB, yb[d] + cell * yst[d], bytes, bar);
-                const double *yl = ylp + cell * FRS, *yu = yup + cell * FRS, *cr = crp + cell * CRS;
-                tma_load_1d(S + L::ylrec, yl, kbytes, bar);
-                tma_load_1d(S + L::ylm, yl + moffK, mbytes, bar);
-                tma_load_1d(S + L::yurec, yu, kbytes, bar);
-                tma_load_1d(S + L::yum, yu + moffK, mbytes, bar);
-                tma_load_1d(S + L::crec, cr, cbytes, bar);
-                tma_load_1d(S + L::cgn, cr + moffC, mbytes, bar);
-                tma_load_1d(S + L::cgp, cr + moffC + NVP, mbytes, bar);
+    // ---- bulk copies (issued by one elected lane): global sources of a step are linear in the cell index
+    constexpr int DJ0 = SGN == 0 ? -2 : (SGN > 0 ? -2 : -1), DJ1 = SGN == 0 ? -1 : (SGN > 0 ? -1 : 1), DJ2 = SGN == 0 ? 1 : (SGN > 0 ? 1 : 2);
+    auto issue_x = [&](int row) {
+        const int sl = (row - rows_first) % NSX;
+        mbar_expect_tx(&bars[sl], bytes);
+        tma_load_1d(ring + sl * QB, xrow_ptr(fcur, A.ghost, row, j) + qa, bytes, &bars[sl]);
+    };
+    // stage of step st: record of x-face st and, for cell st-1, its y-neighbour rows, y-face records and cell record
+    auto issue_stage = [&](int st) {
+        const int sl = (st - c0) & 1;
+        double *S = stages + sl * L::size;
+        uint64_t *bar = &bars[NSX + sl];
+        const bool have_cell = st > c0;
+        mbar_expect_tx(bar, fbytes + (have_cell ? NY * bytes + 2 * fbytes + cbytes : 0));
+        tma_load_1d(S + L::xrec, A.frec0 + ((size_t)j * (GI + 1) + st) * FRS, fbytes, bar);
+        if (have_cell) {
+            const size_t cell = st - 1;
+            int yst;
+            const double *y0p = yrow_base(fcur, A.ghost, j + DJ0, &yst) + qa;
+            tma_load_1d(S + L::yrow, y0p + cell * yst, bytes, bar);
+            const double *y1p = yrow_base(fcur, A.ghost, j + DJ1, &yst) + qa;
+            tma_load_1d(S + L::yrow + QB, y1p + cell * yst, bytes, bar);
+            const double *y2p = yrow_base(fcur, A.ghost, j + DJ2, &yst) + qa;
+            tma_load_1d(S + L::yrow + 2 * QB, y2p + cell * yst, bytes, bar);
+            if (NY == 4) {
+                const double *y3p = yrow_base(fcur, A.ghost, j + 2, &yst) + qa;
+                tma_load_1d(S + L::yrow + 3 * QB, y3p + cell * yst, bytes, bar);
             }
-        };
-
-        if (lead) {
-            for (int i = 0; i < NSX + 2; ++i) mbar_init(&bars[i], 1);
-            mbar_fence_init();
+            const double *yl = A.frec1 + ((size_t)j * GI + cell) * FRS;
+            tma_load_1d(S + L::ylrec, yl, fbytes, bar);
+            tma_load_1d(S + L::yurec, yl + (size_t)GI * FRS, fbytes, bar);
+            tma_load_1d(S + L::crec, A.crec + ((size_t)j * GI + cell) * CRS, cbytes, bar);
         }
-        __syncthreads();
-        if (lead) {
-            for (int row = rows_first; row < rows_first + NSX; ++row) issue_x(row);
-            issue_stage(c0);
-            issue_stage(c0 + 1);
-        }
-        __syncthreads();                                             // rows c0-2, c0-1 consumed
-        if (lead) { issue_x(c0 + 1); issue_x(c0 + 2); }
-        for (int a = c0; a <= c1; ++a) {
-            __syncthreads();                                         // step a done: row a and stage a are free
-            if (lead) {
-                if (a + 3 <= rows_last) issue_x(a + 3);
-                if (a + 2 <= c1) issue_stage(a + 2);
-            }
-        }
-        return;
+    };
+    if (tid == 0) {
+        for (int i = 0; i < NSX + 2; ++i) mbar_init(&bars[i], 1);
+        mbar_fence_init();
+        for (int row = rows_first; row < rows_first + NSX; ++row) issue_x(row);
+        issue_stage(c0);
+        issue_stage(c0 + 1);
     }
     __syncthreads();                                                 // barriers initialised
 
@@ -131,10 +103,10 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     // Per-thread points p: velocity row m = r + p R; byte offsets are thread base + immediates.  A point outside the chunk
     // (the last point when R*NPT > MC, the tail of a ragged chunk) re-reads the chunk's first element; only its store is masked.
     constexpr int QSTEP = R * NU * 8, MSTEP = R * 8;
-    const int qb0 = (qsh + r * NU + k) * 8, mb0 = (msh + r) * 8;
+    const int qb0 = (qsh + r * NU + k) * 8, mb0 = (m0 + r) * 8;
     int qo[NPT], mo[NPT];
 #pragma unroll
-    for (int p = 0; p < NPT; ++p) { qo[p] = r + p * R < mc ? p * QSTEP : qsh * 8 - qb0; mo[p] = r + p * R < mc ? p * MSTEP : msh * 8 - mb0; }
+    for (int p = 0; p < NPT; ++p) { qo[p] = r + p * R < mc ? p * QSTEP : qsh * 8 - qb0; mo[p] = r + p * R < mc ? p * MSTEP : m0 * 8 - mb0; }
 #define QOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * QSTEP : qo[p])
 #define MOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * MSTEP : mo[p])
     double vn[NPT], fm[NPT], fc[NPT], Fprev[NPT];
@@ -156,6 +128,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         for (int p = 0; p < NPT; ++p) { fm[p] = ldsd(ra, QOFF(p)); fc[p] = ldsd(rb, QOFF(p)); }
     }
     __syncthreads();                                                 // rows c0-2, c0-1 consumed
+    if (tid == 0) { issue_x(c0 + 1); issue_x(c0 + 2); }
     // wall flags of the two y-faces (CTA-uniform)
     const bool wl2 = beyond_wall_y(j - 2), wl1 = beyond_wall_y(j - 1), wu1 = beyond_wall_y(j + 1), wu2 = beyond_wall_y(j + 2);
     const bool anyy = wl2 || wl1 || wu1 || wu2;
@@ -169,6 +142,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     xslot_new = (2 + sh) % NSX;
     int xw_slot = 0, xw_phase = 1;                                   // barrier slot / phase of row a+1 (index a+1-rows_first = 3 at a = c0)
     int stage_i = 0, stage_phase = 0;
+    int issuer = 0;                                                  // thread that issues the bulk copies after this step (lane 0 of a rotating warp)
     for (int a = c0; a <= c1; ++a) {                                 // x-face a, then cell a-1
         const unsigned char *S = stages_b + stage_i * (L::size * 8);
         mbar_wait(&bars[NSX + stage_i], stage_phase);
@@ -187,7 +161,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         const double p3 = Ek * xr[FR_C03];
         const double c4 = uk * xr[FR_MT4];
         const double c45 = uk * fma(uk, xr[FR_MT5], sgx * xr[FR_MT4]);
-        const unsigned char *xm = S + L::xm * 8 + mb0;
+        const unsigned char *xm = S + (L::xrec + FR_NCOEF + NUP) * 8 + mb0;
         const unsigned char *rn = ring_b + xslot_new * QBB;
         if (++xslot_new == NSX) xslot_new = 0;
         bool xw0 = false, xw1 = false, xw2 = false, xw3 = false;
@@ -219,7 +193,8 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
             l4 = ylr[FR_MT4]; l5 = ylr[FR_MT5]; u4 = yur[FR_MT4]; u5 = yur[FR_MT5];
         }
         const unsigned char *y0 = S + L::yrow * 8 + qb0, *y1 = y0 + QBB, *y2 = y1 + QBB, *y3 = y2 + QBB;
-        const unsigned char *ylm = S + L::ylm * 8 + mb0, *yum = S + L::yum * 8 + mb0, *cgn = S + L::cgn * 8 + mb0, *cgp = S + L::cgp * 8 + mb0;
+        const unsigned char *ylm = S + (L::ylrec + FR_NCOEF + NUP) * 8 + mb0, *yum = S + (L::yurec + FR_NCOEF + NUP) * 8 + mb0;
+        const unsigned char *cgn = S + (L::crec + CR_NCOEF + 2 * NUP) * 8 + mb0, *cgp = cgn + NVP * 8;
         unsigned char *out = out_row + (size_t)max(a - 1, 0) * (NPAD * 8);
 
         auto body = [&](auto fl) {                                   // fl: some stencil of this step touches a wall
@@ -277,6 +252,12 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         };
         if (anyx || (anyy && have_cell)) body(true_c{}); else body(false_c{});
         __syncthreads();                                             // row a and stage a are consumed
+        if (tid == issuer) {                                         // one lane of warp (a - c0) mod W issues the copies of two steps ahead
+            if (a + 3 <= rows_last) issue_x(a + 3);
+            if (a + 2 <= c1) issue_stage(a + 2);
+        }
+        issuer += 32;
+        if (issuer >= BT) issuer = 0;
     }
 }
 
@@ -284,7 +265,11 @@ static_assert(StageL<3>::BYTES == G_SMEM_UPD3 && StageL<4>::BYTES == G_SMEM_UPD4
 
 // one launch covers the chunk range [chunk0, chunk0 + nch): the CTA dispatches on the sign class of its chunk (the two uniform
 // classes of a cell read its records while they are in the L2)
-extern "C" __global__ void __launch_bounds__(BT + 32, G_MINB_UPD) k_flux_update(const KArgs A, const int chunk0)
+#ifdef UGKS_MINB_UPD                                                // experiment override (UGKS_JIT_DEFS)
+#undef G_MINB_UPD
+#define G_MINB_UPD UGKS_MINB_UPD
+#endif
+extern "C" __global__ void __launch_bounds__(BT, G_MINB_UPD) k_flux_update(const KArgs A, const int chunk0)
 {
     int b = blockIdx.x;
     const int j = b % GJ; b /= GJ;

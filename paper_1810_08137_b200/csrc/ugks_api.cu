@@ -121,7 +121,7 @@ static void choose_R(int kind, int Nu, int cmax, int *R, int *npt)
 static void choose_geometry(int kind, const double *v, int I, int J, int Nu, int Nv, KGeom *G)
 {
     int cm = 800 / Nu; if (cm < 1) cm = 1; if (cm > 56) cm = 56;
-    if (Nu > 128) cm = kind == JIT_MOMENTS ? 14 : 10;                // wide rows: one thread per column (measured, C5)
+    if (Nu > 128) cm = kind == JIT_MOMENTS ? 14 : 5;                 // wide rows: one thread per column (measured, C5)
     make_chunks(v, Nv, Nu, cm, G);
     choose_R(kind, Nu, G->cmax, &G->R, &G->npt);
     int s = 32;

@@ -29,6 +29,7 @@ int pad2i(int x) { return (x + 1) & ~1; }
 int cdivi(int a, int b) { return (a + b - 1) / b; }
 
 // host mirrors of MomL<MIXED>::BYTES and StageL<NY>::BYTES (the device code static_asserts that they agree)
+int nsxm() { const char *e = getenv("UGKS_NSXM"); const int n = e ? atoi(e) : 3; return n < 2 ? 2 : (n > 4 ? 4 : n); }   // x-ring slots of k_cell_moments
 int smem_mom(const UgksParams &P, const KGeom &G, bool mixed)
 {
     const int BT = (P.Nu * G.R + 31) / 32 * 32, QB = pad2i(G.cmax * P.Nu + 1);
@@ -37,8 +38,8 @@ int smem_mom(const UgksParams &P, const KGeom &G, bool mixed)
     int per = P.Nu;
     for (int q = 1; q <= P.Nu; ++q) if (26 * cdivi(lenx, q) + ny * cdivi(P.Nu, q) <= BT) { per = q; break; }
     const int nitem = 26 * cdivi(lenx, per) + ny * cdivi(P.Nu, per), NUS = P.Nu | 1, NROW = G.R * G.npt + 1;
-    const int total = 3 * QB + 4 * QB + (G.R == 1 ? 0 : 2 * NA * BT) + pad2i(2 * NC * NUS) + pad2i(13 * NUS) + pad2i(NROW * 6) +
-                      pad2i(2 * nitem) + 5;
+    const int total = nsxm() * QB + 4 * QB + (G.R == 1 ? 0 : NA * BT) + pad2i(2 * NC * NUS) + pad2i(13 * NUS) + pad2i(NROW * 6) +
+                      pad2i(2 * nitem) + nsxm() + 3;
     return total * 8;
 }
 int smem_upd(const UgksParams &P, const KGeom &G, int ny)
@@ -57,7 +58,8 @@ int min_blocks(int threads, int smem, int regs)
 }
 int threads_of(int kind, const UgksParams &P, const KGeom &G)
 {
-    return (P.Nu * G.R + 31) / 32 * 32 + (kind == JIT_MOMENTS ? 32 : 0);      // k_cell_moments: + the producer warp
+    (void)kind;
+    return (P.Nu * G.R + 31) / 32 * 32;                              // no producer warp: one thread per (column, parallel row)
 }
 
 std::string dir_of_this_library()
@@ -109,7 +111,7 @@ std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const dou
     DEF("G_KXM_END", P.kxm_end); DEF("G_KXP_BEGIN", P.kxp_begin); DEF("G_RAGGED", G.ragged() ? 1 : 0);
     if (kind == JIT_MOMENTS) {
         const int sm_u = smem_mom(P, G, false), sm_m = smem_mom(P, G, true);
-        DEF("G_SMEM_MOM", sm_u); DEF("G_SMEM_MOMX", sm_m);
+        DEF("G_SMEM_MOM", sm_u); DEF("G_SMEM_MOMX", sm_m); DEF("G_NSXM", nsxm());
         DEF("G_MINB_MOM", min_blocks(threads, sm_u, 128)); DEF("G_MINB_MOMX", min_blocks(threads, sm_m, 128));
     } else {
         const int su3 = smem_upd(P, G, 3), su4 = smem_upd(P, G, 4);

@@ -15,10 +15,14 @@
 //     reduction: (1) partial sums to shared memory; (2) sum over the R threads of a column, forming C_b +- B_b for the two
 //     x-sides; (3) balanced work items (output, k-range): dot product over k with the factors wu u^a H(+-u);
 //     (4) one thread per output adds its items and stores.  All job tables of stages 2..4 are compile-time.
+//   * there is no producer warp: after the barrier of step a one lane of a rotating warp issues the bulk copies of the rows
+//     that barrier freed.  The partial sums are single-buffered: an mbarrier ("part free", one arrival per warp after its
+//     stage-2 reads) orders the next cell's stores behind them without a second CTA-wide barrier.
 #pragma once
 #include "ugks_jit_common.cuh"
 
-constexpr int NSXM = 3;                                              // x-ring slots
+constexpr int NSXM = G_NSXM;                                         // x-ring slots (>= 2)
+constexpr int NW = BT / 32;                                          // warps of a CTA
 constexpr int NFAC = 13;                                             // factor tables: 5 (x+), 5 (x-), 3 (y)
 // raw sum idx -> (power of the per-column velocity, column sum) ; x sets: columns 0..2 = C_b +- B_b, 3..5 = B_b
 __constant__ int c_xa[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 2, 3, 4, 2, 2 };
@@ -53,12 +57,12 @@ struct MomL {                                                        // sizes an
     static constexpr int NROW = R * NPT + 1;                         // weight rows incl. zero rows for a ragged chunk
     static constexpr int O_YBUF = NSXM * QB;
     static constexpr int O_PART = O_YBUF + 4 * QB;
-    static constexpr int O_COL = O_PART + (R == 1 ? 0 : 2 * NA * BT);
+    static constexpr int O_COL = O_PART + (R == 1 ? 0 : NA * BT);
     static constexpr int O_FAC = O_COL + pad2c(2 * NC * NUS);
     static constexpr int O_MTAB = O_FAC + pad2c(NFAC * NUS);
     static constexpr int O_IRES = O_MTAB + pad2c(NROW * 6);
     static constexpr int O_BARS = O_IRES + pad2c(2 * NITEM);
-    static constexpr int TOTAL = O_BARS + NSXM + 2;
+    static constexpr int TOTAL = O_BARS + NSXM + 3;
     static constexpr int BYTES = TOTAL * 8;
 };
 
@@ -81,12 +85,12 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
     double *sm = reinterpret_cast<double *>(smem_raw);
     double *xring = sm;                                              // [NSXM][QB]
     double *ybuf = sm + L::O_YBUF;                                   // [2][2][QB]
-    double *part = sm + L::O_PART;                                   // [2][NA][BT]
+    double *part = sm + L::O_PART;                                   // [NA][BT]
     double *col = sm + L::O_COL;                                     // [2][NC][NUS]
     double *fac = sm + L::O_FAC;                                     // [NFAC][NUS]
     double *mtab = sm + L::O_MTAB;                                   // [NROW][6]: w, w v, w v^2, w v^3, w v^4, H(v)
     double *ires = sm + L::O_IRES;                                   // [2][NITEM] stage-3 item results
-    uint64_t *bars = reinterpret_cast<uint64_t *>(sm + L::O_BARS);   // [NSXM] x rows, [2] y stages
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sm + L::O_BARS);   // [NSXM] x rows, [2] y stages, [1] part free
 
     const int tid = threadIdx.x;
     const bool active = tid < NU * R;
@@ -94,44 +98,27 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
     const double *fcur = A.fcur;
     const int rows_first = c0 - 1, rows_last = c1;                   // cells c0-1 .. c1 are staged
 
-    if (tid == 0) {
-        for (int i = 0; i < NSXM + 2; ++i) mbar_init(&bars[i], 1);
-        mbar_fence_init();
-    }
-    if (tid >= BT) {                                                 // ---- producer warp: one lane issues every bulk copy
-        const bool lead = tid == BT;
+    // ---- bulk copies (issued by one elected lane)
+    auto issue_x = [&](int row) {
+        const int sl = (row - rows_first) % NSXM;
+        mbar_expect_tx(&bars[sl], bytes);
+        tma_load_1d(xring + sl * QB, xrow_ptr(fcur, A.ghost, row, j) + qa, bytes, &bars[sl]);
+    };
+    auto issue_y = [&](int cell) {
+        const int buf = (cell - c0) & 1;
         int ystm, ystp;
         const double *ybm = yrow_base(fcur, A.ghost, j - 1, &ystm) + qa, *ybp = yrow_base(fcur, A.ghost, j + 1, &ystp) + qa;
-        auto issue_x = [&](int row) {
-            const int sl = (row - rows_first) % NSXM;
-            mbar_expect_tx(&bars[sl], bytes);
-            tma_load_1d(xring + sl * QB, xrow_ptr(fcur, A.ghost, row, j) + qa, bytes, &bars[sl]);
-        };
-        auto issue_y = [&](int cell) {
-            const int buf = (cell - c0) & 1;
-            mbar_expect_tx(&bars[NSXM + buf], 2 * bytes);
-            tma_load_1d(ybuf + (buf * 2) * QB, ybm + (size_t)cell * ystm, bytes, &bars[NSXM + buf]);
-            tma_load_1d(ybuf + (buf * 2 + 1) * QB, ybp + (size_t)cell * ystp, bytes, &bars[NSXM + buf]);
-        };
-        __syncthreads();                                             // barriers initialised, tables written
-        if (lead) {
-            for (int row = rows_first; row < rows_first + NSXM && row <= rows_last; ++row) issue_x(row);
-            issue_y(c0);
-            if (c0 + 1 < c1) issue_y(c0 + 1);
-        }
-        __syncthreads();                                             // rows c0-1, c0 consumed
-        if (lead) {
-            if (c0 + 2 <= rows_last) issue_x(c0 + 2);
-            if (c0 + 3 <= rows_last) issue_x(c0 + 3);
-        }
-        for (int a = c0; a < c1 + 3; ++a) {
-            __syncthreads();                                         // step a done: row a+1 and y stage a are free
-            if (lead && a < c1) {
-                if (a + 4 <= rows_last) issue_x(a + 4);
-                if (a + 2 < c1) issue_y(a + 2);
-            }
-        }
-        return;
+        mbar_expect_tx(&bars[NSXM + buf], 2 * bytes);
+        tma_load_1d(ybuf + (buf * 2) * QB, ybm + (size_t)cell * ystm, bytes, &bars[NSXM + buf]);
+        tma_load_1d(ybuf + (buf * 2 + 1) * QB, ybp + (size_t)cell * ystp, bytes, &bars[NSXM + buf]);
+    };
+    if (tid == 0) {
+        for (int i = 0; i < NSXM + 2; ++i) mbar_init(&bars[i], 1);
+        mbar_init(&bars[NSXM + 2], NW);
+        mbar_fence_init();
+        for (int row = rows_first; row < rows_first + NSXM && row <= rows_last; ++row) issue_x(row);
+        issue_y(c0);
+        if (c0 + 1 < c1) issue_y(c0 + 1);
     }
     for (int i = tid; i < NU; i += BT) {
         const double u = c_u[i], w = c_wu[i];
@@ -214,15 +201,24 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
         }
     }
     __syncthreads();                                                 // rows c0-1, c0 consumed
+    if (tid == 0) {
+        if (rows_first + NSXM <= rows_last) issue_x(rows_first + NSXM);
+        if (rows_first + NSXM + 1 <= rows_last) issue_x(rows_first + NSXM + 1);
+    }
     const bool ym_miss = beyond_wall_y(j - 1), yp_miss = beyond_wall_y(j + 1);
     const double sy = ch.z > 0 ? 1.0 : -1.0;                         // side of the y-contribution (uniform chunks)
-    constexpr int s3lag = R == 1 ? 1 : 2;                            // pipeline lag of stage 3 behind stage 1
+    // pipeline of one iteration a: stage 1 (cell a) -> [wait "part free"] store partials -> BARRIER -> (elected lane: bulk
+    // copies of the freed slots) -> stage 2 (cell a) -> stage 3 (cell a - LAG3) -> stage 4 (cell a - LAG3 - 1)
+    constexpr int LAG3 = R == 1 ? 0 : 1;
+    uint64_t *pfree = &bars[NSXM + 2];
+    const int lane = tid & 31;
     constexpr int NXJ = 3 * NU, NYJ = (NA - 6) * NU;                 // stage-2 jobs: (b, k) x-jobs, (i, k) y-jobs
     constexpr int S2X = cdiv(NXJ, BT), S2Y = cdiv(NYJ, BT);
     double *cmom_row = A.cmom + ((size_t)j * GI * NCHUNK + chunk) * CMS;
 
-    int xslot = 2, xphase = 0, ybuf_i = 0, yphase = 0;               // ring slot / phase of row a+1 and of y stage a
-    for (int a = c0; a < c1 + 3; ++a) {
+    int xslot = 2 % NSXM, xphase = 2 / NSXM, ybuf_i = 0, yphase = 0; // ring slot / phase of row a+1 and of y stage a
+    int issuer = 0;                                                  // lane 0 of a rotating warp issues the copies of a step
+    for (int a = c0; a < c1 + LAG3 + 1; ++a) {
         if (a < c1) {                                                // stage 1: point sums of cell a
             mbar_wait(&bars[xslot], xphase);                         // row a+1
             mbar_wait(&bars[NSXM + ybuf_i], yphase);
@@ -282,14 +278,22 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
                     for (int i = 6; i < NA; ++i) cc[(3 + i) * NUS] = acc[i];
                 }
             } else {
-                double *pp = part + (a & 1) * NA * BT + tid;
+                if (a > c0) mbar_wait(pfree, (a - c0 - 1) & 1);      // every warp has read the partials of cell a-1
+                double *pp = part + tid;
 #pragma unroll
                 for (int i = 0; i < NA; ++i) pp[i * BT] = acc[i];
             }
         }
-        if (R > 1 && a - 1 >= c0 && a - 1 < c1) {                    // stage 2: column sums of cell a-1
-            const double *pp = part + ((a - 1) & 1) * NA * BT;
-            double *cc = col + ((a - 1) & 1) * NC * NUS;
+        __syncthreads();                                             // partials of cell a complete; row a+1 and y stage a consumed
+        if (tid == issuer && a < c1) {
+            if (a + 1 + NSXM <= rows_last) issue_x(a + 1 + NSXM);
+            if (a + 2 < c1) issue_y(a + 2);
+        }
+        issuer += 32;
+        if (issuer >= BT) issuer = 0;
+        if (R > 1 && a < c1) {                                       // stage 2: column sums of cell a
+            const double *pp = part;
+            double *cc = col + (a & 1) * NC * NUS;
 #pragma unroll
             for (int q = 0; q < S2X; ++q) {                          // x, power b of t: C_b +- B_b for the two sides, B_b
                 const int g = tid + q * BT;
@@ -303,6 +307,7 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
                     o[0] = C + Bs; o[3 * NUS] = C - Bs; o[6 * NUS] = Bs;
                 }
             }
+            double ysum[S2Y];
 #pragma unroll
             for (int q = 0; q < S2Y; ++q) {                          // y sums
                 const int g = tid + q * BT;
@@ -312,11 +317,18 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
                     double S = pa[0];
 #pragma unroll
                     for (int rr = 1; rr < R; ++rr) S += pa[rr * NU];
-                    cc[(9 + iq) * NUS + kk] = S;
+                    ysum[q] = S;
                 }
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(pfree);                       // this warp is done with the partials
+#pragma unroll
+            for (int q = 0; q < S2Y; ++q) {
+                const int g = tid + q * BT;
+                if (g < NYJ) { const int iq = g / NU, kk = g - iq * NU; cc[(9 + iq) * NUS + kk] = ysum[q]; }
+            }
         }
-        const int c3 = a - s3lag, c4 = c3 - 1;
+        const int c3 = a - LAG3, c4 = c3 - 1;
         if (c3 >= c0 && c3 < c1) {                                   // stage 3: items (output, k-range) of cell c3
             const unsigned char *cc = reinterpret_cast<const unsigned char *>(col + (c3 & 1) * NC * NUS);
             const unsigned char *fb = reinterpret_cast<const unsigned char *>(fac);
@@ -341,12 +353,13 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
                 if (v < NOUT) {
                     const int ns = v < 2 * NRAW ? L::NSX : L::NSY;
                     double sum = ir[o_first[q]];
-                    for (int h = 1; h < ns; ++h) sum += ir[o_first[q] + h];
+#pragma unroll
+                    for (int h = 1; h < cmaxi(L::NSX, L::NSY); ++h)
+                        if (h < ns) sum += ir[o_first[q] + h];
                     dst[o_dst[q]] = sum;
                 }
             }
         }
-        __syncthreads();                                             // row a+1 is consumed by every thread
     }
 }
 
@@ -356,12 +369,12 @@ static_assert(MomL<false>::BYTES == G_SMEM_MOM && MomL<true>::BYTES == G_SMEM_MO
 #undef G_MINB_MOM
 #define G_MINB_MOM UGKS_MINB_MOM
 #endif
-extern "C" __global__ void __launch_bounds__(BT + 32, G_MINB_MOM) k_cell_moments(const KArgs A, const int chunk0)
+extern "C" __global__ void __launch_bounds__(BT, G_MINB_MOM) k_cell_moments(const KArgs A, const int chunk0)
 {
     cell_moments_body<false>(A, chunk0);
 }
 #if G_NMIX > 0
-extern "C" __global__ void __launch_bounds__(BT + 32, G_MINB_MOMX) k_cell_moments_mixed(const KArgs A, const int chunk0)
+extern "C" __global__ void __launch_bounds__(BT, G_MINB_MOMX) k_cell_moments_mixed(const KArgs A, const int chunk0)
 {
     cell_moments_body<true>(A, chunk0);
 }

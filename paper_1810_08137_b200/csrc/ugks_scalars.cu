@@ -420,48 +420,53 @@ int launch_setup(const UgksParams &P, const double *bc_prims, double *ghost, dou
 // ---------------------------------------------------------------------------------------------
 // k_tables: every exponential of the step (S6 and the two cell equilibria of U2), once per face / cell and node:
 // exp(-lam ((u-U)^2 + (v-V)^2)) = E_k[k] E_m[m] on the tensor-product grid, so a face needs Nu + Nv exponentials, not Nu Nv.
-// One thread per table entry; the records are read back by k_flux_update through TMA.
+// One thread per table entry; a block owns TPB consecutive tables (a face Maxwellian, g^n of a cell, g^{n+1} of a cell), so
+// the entry -> (table, node) split is 32-bit arithmetic on small numbers and the stores of a warp are contiguous.  The
+// records are read back by k_flux_update through TMA.
+constexpr int TPB = 16;                                              // tables per block
 __global__ void __launch_bounds__(256) k_tables(const UgksParams P)
 {
-    const int nt = P.NuP + P.NvP;                                    // entries per Maxwellian
+    const unsigned nt = P.NuP + P.NvP;                               // entries per Maxwellian
     const long nfx = nfaces_x(P), nfy = nfaces_y(P), ncell = (long)P.I * P.J;
-    const long total = (nfx + nfy + 2 * ncell) * nt;
-#pragma unroll 4
-    for (long g = (long)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (long)gridDim.x * blockDim.x) {
-        const long rec = g / nt;
-        const int e = (int)(g - rec * nt);
-        const bool isk = e < P.NuP;
-        const int idx = isk ? e : e - P.NuP;
-        const bool pad = isk ? idx >= P.Nu : idx >= P.Nv;
-        const double node = pad ? 0.0 : (isk ? P.u[idx] : P.v[idx]);
-        double lam, cen, pref = 1.0, *dst;
-        bool zero = pad;
-        if (rec < nfx + nfy) {                                       // face Maxwellian (local frame: U normal, V tangential)
-            const int dir = rec >= nfx;
-            double *fr = P.frec[dir] + (dir ? rec - nfx : rec) * P.frs;
-            lam = fr[FR_LAM];
-            cen = (isk == (dir == 0)) ? fr[FR_U] : fr[FR_V];         // x-face: u is normal; y-face: v is normal
-            zero = zero || fr[FR_TYPE] != 0.0;                       // wall faces carry no equilibrium part
-            dst = fr + FR_NCOEF + e;
-        } else {                                                     // cell equilibria g^n (w = 0), g^{n+1} (w = 1)
-            const long cw = rec - nfx - nfy, cell = cw >> 1;
-            const int w = (int)(cw & 1);
-            double *cr = P.crec + cell * P.crs;
-            lam = cr[w ? CR_LP : CR_LN];
-            cen = isk ? cr[w ? CR_UP : CR_UN] : cr[w ? CR_VP : CR_VN];
-            if (isk) pref = cr[w ? CR_GP : CR_GN];
-            dst = cr + CR_NCOEF + (isk ? w * P.NuP + idx : 2 * P.NuP + w * P.NvP + idx);
+    const long total = nfx + nfy + 2 * ncell;
+    for (long rec0 = (long)blockIdx.x * TPB; rec0 < total; rec0 += (long)gridDim.x * TPB) {
+        for (unsigned i = threadIdx.x; i < TPB * nt; i += blockDim.x) {
+            const unsigned rl = i / nt, e = i - rl * nt;
+            const long rec = rec0 + rl;
+            if (rec >= total) break;
+            const bool isk = e < (unsigned)P.NuP;
+            const int idx = isk ? e : e - P.NuP;
+            const bool pad = isk ? idx >= P.Nu : idx >= P.Nv;
+            const double node = pad ? 0.0 : (isk ? P.u[idx] : P.v[idx]);
+            double lam, cen, pref = 1.0, *dst;
+            bool zero = pad;
+            if (rec < nfx + nfy) {                                   // face Maxwellian (local frame: U normal, V tangential)
+                const int dir = rec >= nfx;
+                double *fr = P.frec[dir] + (dir ? rec - nfx : rec) * P.frs;
+                lam = fr[FR_LAM];
+                cen = (isk == (dir == 0)) ? fr[FR_U] : fr[FR_V];     // x-face: u is normal; y-face: v is normal
+                zero = zero || fr[FR_TYPE] != 0.0;                   // wall faces carry no equilibrium part
+                dst = fr + FR_NCOEF + e;
+            } else {                                                 // cell equilibria g^n (w = 0), g^{n+1} (w = 1)
+                const long cw = rec - nfx - nfy, cell = cw >> 1;
+                const int w = (int)(cw & 1);
+                double *cr = P.crec + cell * P.crs;
+                lam = cr[w ? CR_LP : CR_LN];
+                cen = isk ? cr[w ? CR_UP : CR_UN] : cr[w ? CR_VP : CR_VN];
+                if (isk) pref = cr[w ? CR_GP : CR_GN];
+                dst = cr + CR_NCOEF + (isk ? w * P.NuP + idx : 2 * P.NuP + w * P.NvP + idx);
+            }
+            const double d = node - cen;
+            *dst = zero ? 0.0 : pref * exp(-lam * d * d);
         }
-        const double d = node - cen;
-        *dst = zero ? 0.0 : pref * exp(-lam * d * d);
     }
 }
 
 int launch_tables(const UgksParams &P, cudaStream_t st)
 {
-    const long total = ((long)nfaces_x(P) + nfaces_y(P) + 2L * P.I * P.J) * (P.NuP + P.NvP);
-    long blocks = (total + 255) / 256;
-    if (blocks > 148L * 64) blocks = 148L * 64;
+    const long total = (long)nfaces_x(P) + nfaces_y(P) + 2L * P.I * P.J;
+    long blocks = (total + TPB - 1) / TPB;
+    if (blocks > 148L * 128) blocks = 148L * 128;
     k_tables<<<(int)blocks, 256, 0, st>>>(P);
     return 1;
 }

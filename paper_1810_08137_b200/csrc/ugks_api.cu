@@ -76,12 +76,17 @@ static void make_chunks(const double *v, int Nv, int Nu, int cm_target, KGeom *G
     std::vector<int4> tmp;
     int nruns = 0;
     bool fallback = false;
+    // a single v = 0 row directly followed by the v > 0 run joins that run as its first row (flag .w of its first chunk): the
+    // y-fluxes of that row vanish (n = 0) and its half-range sums need one extra per-thread sum in k_cell_moments (ZROW)
+    int zrow = -1;
+    for (int m = 0; m + 1 < Nv; ++m)
+        if (v[m] == 0.0 && v[m + 1] > 0.0 && (m == 0 || v[m - 1] < 0.0)) zrow = m;
     for (int m = 0; m < Nv && !fallback;) {
-        const int sg = v[m] > 0.0 ? 1 : (v[m] < 0.0 ? -1 : 0);
+        const int sg = (v[m] > 0.0 || m == zrow) ? 1 : (v[m] < 0.0 ? -1 : 0);
         int e = m + 1;
         while (e < Nv && (v[e] > 0.0 ? 1 : (v[e] < 0.0 ? -1 : 0)) == sg) ++e;
         const int len = e - m, parts = (len + cm_target - 1) / cm_target, rows = (len + parts - 1) / parts;
-        for (int p0 = m; p0 < e; p0 += rows) tmp.push_back(make_int4(p0, (p0 + rows <= e ? rows : e - p0), sg, 0));
+        for (int p0 = m; p0 < e; p0 += rows) tmp.push_back(make_int4(p0, (p0 + rows <= e ? rows : e - p0), sg, p0 == zrow ? 1 : 0));
         m = e;
         if (++nruns > 8) fallback = true;                            // unsorted nodes: do not shred the grid
     }
@@ -124,9 +129,30 @@ static void choose_geometry(int kind, const double *v, int I, int J, int Nu, int
     if (Nu > 128) cm = kind == JIT_MOMENTS ? 14 : 5;                 // wide rows: one thread per column (measured, C5)
     make_chunks(v, Nv, Nu, cm, G);
     choose_R(kind, Nu, G->cmax, &G->R, &G->npt);
-    int s = 32;
-    while (s > 4 && (long)J * ((I + s - 1) / s) * G->nchunk() < 148L * 8) s >>= 1;
-    G->strip = s;
+    G->strip = 0;                                                    // 0 = automatic (default_strip / choose_strip in apply_geometry)
+    (void)I; (void)J;
+}
+
+static int default_strip(int I) { const int ns = (I + 31) / 32; return (I + ns - 1) / ns; }     // balanced strips of <= 32 cells
+
+// Cells per CTA march.  A march of s cells costs about s + 3 cell times (pipeline fill, the extra stencil rows), so long
+// strips amortise best -- but the CTAs of a launch run in waves of (CTAs per SM) x (SMs), and on paper-sized meshes a launch
+// is only a few waves: then the serial march of a CTA and the partly filled last wave decide (M4-29 at s = 32: 800 CTAs
+// against 740 resident; measured 0.315 ms per step against 0.255 at s = 8).  Rule from the sweeps (C1, C2, M4-29, M3-49,
+// M4-69): the longest balanced strip of at most 32 cells that still gives 4 waves, not below 8 cells (4 when even that
+// leaves the GPU under one wave).
+static int choose_strip(int I, int J, int nchunk, int ctas_per_sm, int sms, int s0)
+{
+    const long cap = (long)ctas_per_sm * sms, per_column = (long)J * nchunk;
+    long ns = (4 * cap + per_column - 1) / per_column;               // strips per row for 4 waves
+    if (ns < 1) ns = 1;
+    int s = (int)((I + ns - 1) / ns);
+    if (s >= s0) return s0;
+    const int smin = per_column * ((I + 7) / 8) < cap ? 4 : 8;
+    if (s < smin) s = smin;
+    if (s > I) s = I;
+    const int nsb = (I + s - 1) / s;                                 // balance the strips
+    return (I + nsb - 1) / nsb;
 }
 
 struct Layout {
@@ -190,7 +216,7 @@ static const char *check_geometry(int kind, const UgksParams &T, const KGeom &G)
 {
     if (G.nchunk() < 1 || G.nchunk() > MAXCHUNK) return "bad chunk count";
     if (G.npt < 1 || G.npt > 16 || G.R < 1 || T.Nu * G.R > 256 || G.R * G.npt < G.cmax) return "R / points per thread out of range";
-    if (G.strip < 1 || G.strip > 4096) return "strip out of range";
+    if (G.strip < 0 || G.strip > T.I) return "strip out of range (0 = automatic, else 1..I)";
     if (jit_smem(kind, T, G) > 227 * 1024) return "chunk does not fit in shared memory";
     return nullptr;
 }
@@ -207,13 +233,30 @@ static int apply_geometry(ugks_ctx *c, int kind, const KGeom &G)
     drop_graph(c);
     JitKernel *jk = nullptr;
     char msg[240];
-    if (jit_get(kind, T, G, c->uhost, c->wuhost, c->vhost, c->wvhost, &jk, msg, sizeof msg)) return fail(c, UGKS_ECUDA, "%s", msg);
+    KGeom Gs = G;
+    const bool auto_strip = Gs.strip == 0;
+    if (auto_strip) Gs.strip = default_strip(T.I);
+    if (jit_get(kind, T, Gs, c->uhost, c->wuhost, c->vhost, c->wvhost, &jk, msg, sizeof msg)) return fail(c, UGKS_ECUDA, "%s", msg);
+    if (auto_strip) {                                                // few waves: pick the strip from this kernel's occupancy, re-compile
+        int sms = 148;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+        const int s = choose_strip(T.I, T.J, G.nchunk(), jit_ctas_per_sm(jk), sms, Gs.strip);
+        if (s != Gs.strip) {
+            Gs.strip = s;
+            if (jit_get(kind, T, Gs, c->uhost, c->wuhost, c->vhost, c->wvhost, &jk, msg, sizeof msg)) return fail(c, UGKS_ECUDA, "%s", msg);
+        }
+    }
+    const KGeom &G2 = Gs;
+    if (getenv("UGKS_DEBUG"))
+        fprintf(stderr, "ugks: %s geometry: %d chunks (cmax %d), R %d, %d points/thread, strip %d, %d CTAs/SM, %d threads, %zu B smem\n",
+                kind == JIT_MOMENTS ? "k_cell_moments" : "k_flux_update", G.nchunk(), G.cmax, G.R, G.npt, G2.strip, jit_ctas_per_sm(jk), jk->threads,
+                jit_smem(kind, T, G));
     if (kind == JIT_MOMENTS) {
         CK(cudaMemcpy(c->chunks_dev, G.chunks.data(), sizeof(int4) * G.nchunk(), cudaMemcpyHostToDevice), "apply_geometry");
-        T.nchunk = G.nchunk(); T.nneg = G.nneg; T.npos = G.npos; T.nmix = G.nmix; T.cmax = G.cmax; T.R = G.R; T.npt = G.npt; T.strip = G.strip;
+        T.nchunk = G.nchunk(); T.nneg = G.nneg; T.npos = G.npos; T.nmix = G.nmix; T.cmax = G.cmax; T.R = G.R; T.npt = G.npt; T.strip = G2.strip;
         c->P = T;
-        *c->gm = G; c->km = jk;
-    } else { *c->gu = G; c->ku = jk; }
+        *c->gm = G2; c->km = jk;
+    } else { *c->gu = G2; c->ku = jk; }
     return UGKS_OK;
 }
 
@@ -238,6 +281,7 @@ int ugks_jit_check(const ugks_mesh *m, const ugks_vgrid *vg, const ugks_bcs *bcs
     for (int kind = 0; kind < 2; ++kind) {
         KGeom G;
         choose_geometry(kind, vg->v, T.I, T.J, T.Nu, T.Nv, &G);
+        G.strip = default_strip(T.I);
         if (const char *why = check_geometry(kind, T, G)) return fail(nullptr, UGKS_EINVAL, "%s", why);
         std::vector<char> cubin;
         std::string out;
@@ -391,14 +435,15 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
             for (int kind = 0; kind < 2; ++kind) {
                 if ((kind == JIT_MOMENTS && only_u) || (kind == JIT_UPDATE && only_m)) continue;
                 KGeom G = kind == JIT_MOMENTS ? *c->gm : *c->gu;
-                if (!strcmp(base, "strip")) G.strip = value;
+                if (!strcmp(base, "strip")) { if (value < 0 || value > P.I) return fail(c, UGKS_EINVAL, "%s", "strip out of range"); G.strip = value; }
                 else if (!strcmp(base, "R")) {
                     if (value < 1 || P.Nu * value > 256) return fail(c, UGKS_EINVAL, "%s", "R out of range");
-                    G.R = value; G.npt = (G.cmax + value - 1) / value;
+                    G.R = value; G.npt = (G.cmax + value - 1) / value; G.strip = 0;
                 } else {                                             // re-chunk with at most `value` rows per chunk
                     if (value < 1 || value > 56) return fail(c, UGKS_EINVAL, "%s", "chunk rows out of range");
                     make_chunks(c->vhost, P.Nv, P.Nu, value, &G);
                     choose_R(kind, P.Nu, G.cmax, &G.R, &G.npt);
+                    G.strip = 0;
                 }
                 const int rc = apply_geometry(c, kind, G);
                 if (rc) return rc;

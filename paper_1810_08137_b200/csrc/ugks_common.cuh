@@ -49,7 +49,7 @@ struct UgksParams {
     const double *Wb;                // [4][4]   cons(prim_b) of FIXED sides
     const double *wallG;             // [4][4]   sum_{outgoing} w n psi_loc g_w per wall side (local frame)
     const double *ghostmom;          // [4][NRAW] half-range raw moments of the ghost row toward the domain (FIXED sides)
-    const int4 *chunks;              // [nchunk] (m0, mc, sign of v over the chunk: +1 / -1 / 0 = mixed, 0)
+    const int4 *chunks;              // [nchunk] (m0, mc, sign of v over the chunk: +1 / -1 / 0 = mixed, 1 if row m0 is a v = 0 row of a +1 chunk)
     double *f[2];                    // ping-pong copies of f, rows padded to Npad
     double *W[2];                    // ping-pong copies of W [cells][4]
     double *cmom;                    // [cells][nchunk][NSET][NRAW]

@@ -33,7 +33,9 @@ int nsxm() { const char *e = getenv("UGKS_NSXM"); const int n = e ? atoi(e) : 3;
 int smem_mom(const UgksParams &P, const KGeom &G, bool mixed)
 {
     const int BT = (P.Nu * G.R + 31) / 32 * 32, QB = pad2i(G.cmax * P.Nu + 1);
-    const int NA = mixed ? 20 : 13, NC = mixed ? 23 : 16, ny = mixed ? 26 : 13;
+    bool zrow = false;
+    for (const int4 &c : G.chunks) if (c.w) zrow = true;
+    const int NA = mixed ? 20 : (zrow ? 14 : 13), NC = mixed ? 23 : (zrow ? 17 : 16), ny = mixed ? 26 : (zrow ? 16 : 13);
     const int lenx = P.kxm_end > P.Nu - P.kxp_begin ? P.kxm_end : P.Nu - P.kxp_begin;
     int per = P.Nu;
     for (int q = 1; q <= P.Nu; ++q) if (26 * cdivi(lenx, q) + ny * cdivi(P.Nu, q) <= BT) { per = q; break; }
@@ -108,6 +110,7 @@ std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const dou
     DEF("G_FRS", P.frs); DEF("G_CRS", P.crs);
     DEF("G_BC0", P.bc[0]); DEF("G_BC1", P.bc[1]); DEF("G_BC2", P.bc[2]); DEF("G_BC3", P.bc[3]);
     DEF("G_NCHUNK", G.nchunk()); DEF("G_NMIX", G.nmix); DEF("G_MC", G.cmax); DEF("G_R", G.R); DEF("G_NPT", G.npt); DEF("G_STRIP", G.strip);
+    { int z = 0; for (const int4 &c : G.chunks) if (c.w) z = 1; DEF("G_HAS_ZROW", z); }
     DEF("G_KXM_END", P.kxm_end); DEF("G_KXP_BEGIN", P.kxp_begin); DEF("G_RAGGED", G.ragged() ? 1 : 0);
     if (kind == JIT_MOMENTS) {
         const int sm_u = smem_mom(P, G, false), sm_m = smem_mom(P, G, true);
@@ -120,7 +123,7 @@ std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const dou
     }
 #undef DEF
     s += "__constant__ int4 c_chunks[] = {";
-    for (int i = 0; i < G.nchunk(); ++i) { snprintf(b, sizeof b, "%s{%d, %d, %d, 0}", i ? ", " : "", G.chunks[i].x, G.chunks[i].y, G.chunks[i].z); s += b; }
+    for (int i = 0; i < G.nchunk(); ++i) { snprintf(b, sizeof b, "%s{%d, %d, %d, %d}", i ? ", " : "", G.chunks[i].x, G.chunks[i].y, G.chunks[i].z, G.chunks[i].w); s += b; }
     s += "};\n";
     if (const char *extra = getenv("UGKS_JIT_DEFS")) { s += extra; s += "\n"; }      // developer aid: extra #define lines for experiments
     add_doubles(s, "c_u", u, P.Nu); add_doubles(s, "c_wu", wu, P.Nu); add_doubles(s, "c_v", v, P.Nv); add_doubles(s, "c_wv", wv, P.Nv);
@@ -186,6 +189,14 @@ int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, cons
     if (e != cudaSuccess) { snprintf(err, errlen, "shared-memory opt-in failed: %s", cudaGetErrorString(e)); return 1; }
     *out = m;
     return 0;
+}
+
+// CTAs of this kernel that one SM holds (registers, shared memory, threads) on the current device
+int jit_ctas_per_sm(const JitKernel *m)
+{
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, (const void *)m->k, m->threads, (size_t)m->smem) != cudaSuccess) { cudaGetLastError(); return 1; }
+    return n < 1 ? 1 : n;
 }
 
 static KArgs_h make_args(const UgksParams &P, int cur)

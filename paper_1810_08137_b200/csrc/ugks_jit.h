@@ -34,5 +34,6 @@ int jit_compile(int kind, const std::string &prelude, std::vector<char> *cubin, 
 // kernel for this geometry (compiled once per process and prelude); sets the shared-memory opt-in on the current device
 int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, const double *wu, const double *v, const double *wv,
             JitKernel **out, char *err, size_t errlen);
+int jit_ctas_per_sm(const JitKernel *m);
 int jit_launch_cell_moments(const JitKernel *m, const UgksParams &P, const KGeom &G, int cur, cudaStream_t st);
 int jit_launch_flux_update(const JitKernel *m, const UgksParams &P, const KGeom &G, int cur, cudaStream_t st);

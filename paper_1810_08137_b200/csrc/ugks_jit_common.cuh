@@ -34,6 +34,7 @@ constexpr int QBB = QB * 8;
 
 // per-(cell, chunk) half-range raw moment sets (see ugks_common.cuh): sets 0 = x+, 1 = x-, 2 = y+, 3 = y-
 constexpr int NSET = 4, NRAW = 13, CMS = NSET * NRAW;
+enum { RW_M00 = 0, RW_M10, RW_M20, RW_M30, RW_M01, RW_M11, RW_M02, RW_M12, RW_S20, RW_S30, RW_S40, RW_S21, RW_S22 };
 // face / cell record layout (see ugks_common.cuh)
 constexpr int FR_NCOEF = 24;
 enum { FR_LAM = 0, FR_U = 1, FR_V = 2, FR_TYPE = 3, FR_RHOW = 4, FR_MT4 = 5, FR_MT5 = 6, FR_TAU = 7, FR_C00 = 8, FR_C01 = 9,

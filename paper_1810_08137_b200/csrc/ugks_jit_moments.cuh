@@ -34,9 +34,14 @@ constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
 constexpr int cmaxi(int a, int b) { return a > b ? a : b; }
 // stage-3 split: the fewest columns per item such that all items (26 x-outputs over ~Nu/2 columns, the y-outputs over Nu
 // columns) fit one pass of the CTA's compute threads; one item per output if even that does not fit
+// A sorted grid with a node v = 0 (odd grids, AMB-5: H(0) = 1/2) keeps that row as the FIRST row of the first v > 0 chunk
+// (chunk flag .w): all its y-sums with a power of n vanish, so besides the half weight in A_0 of the y+ set it only adds
+// sum w/2 (f_c - h sigma) to M00, M01, M02 of the y- set: one more per-thread sum, column and three outputs (ZROW).
+constexpr bool ZROW = G_HAS_ZROW != 0;
+constexpr int NYX = ZROW ? 3 : 0;                                    // extra y- outputs of the chunk that holds the v = 0 row
 constexpr int s3_per(bool mixed)
 {
-    const int lenx = cmaxi(KXM_END, NU - KXP_BEGIN), ny = mixed ? 2 * NRAW : NRAW;
+    const int lenx = cmaxi(KXM_END, NU - KXP_BEGIN), ny = mixed ? 2 * NRAW : NRAW + NYX;
     for (int per = 1; per <= NU; ++per)
         if (2 * NRAW * cdiv(lenx, per) + ny * cdiv(NU, per) <= BT) return per;
     return NU;
@@ -44,15 +49,15 @@ constexpr int s3_per(bool mixed)
 
 template <bool MIXED>
 struct MomL {                                                        // sizes and the shared-memory carve-up (offsets in doubles)
-    static constexpr int NA = MIXED ? 20 : 13;                       // per-thread sums: 6 (x) + 7 (y) [+ 7 (y-)]
-    static constexpr int NC = MIXED ? 23 : 16;                       // columns after stage 2: 9 (x) + 7 (y) [+ 7]
-    static constexpr int NOUT = MIXED ? 4 * NRAW : 3 * NRAW;
-    static constexpr int NYS = MIXED ? 2 : 1;                        // y sets written by a chunk
+    static constexpr int NA = MIXED ? 20 : (ZROW ? 14 : 13);         // per-thread sums: 6 (x) + 7 (y) [+ 7 (y-) | + 1 (v = 0 row)]
+    static constexpr int NC = MIXED ? 23 : (ZROW ? 17 : 16);         // columns after stage 2: 9 (x) + 7 (y) [+ 7 | + 1]
+    static constexpr int NYO = MIXED ? 2 * NRAW : NRAW + NYX;        // y outputs of a chunk
+    static constexpr int NOUT = 2 * NRAW + NYO;
     static constexpr int LENX = cmaxi(KXM_END, NU - KXP_BEGIN);
     static constexpr int PER = s3_per(MIXED);
     static constexpr int NSX = cdiv(LENX, PER), NSY = cdiv(NU, PER);
     static constexpr int PERX = cdiv(LENX, NSX), PERY = cdiv(NU, NSY);
-    static constexpr int NITEM = 2 * NRAW * NSX + NYS * NRAW * NSY;
+    static constexpr int NITEM = 2 * NRAW * NSX + NYO * NSY;
     static constexpr int NUS = NU | 1;                               // odd column stride
     static constexpr int NROW = R * NPT + 1;                         // weight rows incl. zero rows for a ragged chunk
     static constexpr int O_YBUF = NSXM * QB;
@@ -77,7 +82,9 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
     const int s = b % NSTRIP;
     const int chunk = chunk0 + b / NSTRIP;                           // chunks are sorted: [v < 0][v > 0][mixed]
     const int4 ch = c_chunks[chunk];
-    const int c0 = s * STRIP, c1 = min(c0 + STRIP, GI);              // cells [c0, c1)
+    // every CTA marches exactly STRIP cells (a compile-time trip count): the last strip of a row that STRIP does not divide
+    // starts at GI - STRIP and re-computes a few cells of its neighbour (same inputs, same arithmetic, same bits)
+    const int c0 = min(s * STRIP, GI - STRIP), c1 = c0 + STRIP;      // cells [c0, c1)
     const int m0 = ch.x, mc = ch.y;
     const int q0 = m0 * NU, qa = q0 & ~1, qsh = q0 - qa;             // 16-byte aligned copy start; shift of the chunk inside
     const uint32_t bytes = (uint32_t)(pad2c(mc * NU + qsh) * 8);
@@ -136,7 +143,8 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
         const double v = in ? c_v[m0 + i] : 0.0, w = in ? c_wv[m0 + i] : 0.0;
         double *o = mtab + i * 6;
         o[0] = w; o[1] = w * v; o[2] = w * v * v; o[3] = w * v * v * v; o[4] = w * v * v * v * v;
-        o[5] = v > 0.0 ? 1.0 : (v < 0.0 ? 0.0 : 0.5);
+        // MIXED: H(v) (AMB-5); uniform chunks: the weight of A_0, w (w/2 on a v = 0 row: the other half goes to the y- set)
+        o[5] = MIXED ? (v > 0.0 ? 1.0 : (v < 0.0 ? 0.0 : 0.5)) : (in && v == 0.0 ? 0.5 * w : w);
     }
     // stage-3 work items of this thread: item = (output v = (set, idx), part h of its k-range); x+ sums u_k >= 0, x- sums u_k <= 0
     constexpr int S3R = cdiv(NITEM, BT);
@@ -152,10 +160,16 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
             ci = c < 3 ? (set == 0 ? c : 3 + c) : 3 + c;             // columns: 0..2 C+B, 3..5 C-B, 6..8 B
             kb = set == 0 ? KXP_BEGIN : 0; ke = set == 0 ? NU : KXM_END;
         } else if (it < NITEM) {
-            const int w = it - 2 * NRAW * L::NSX, v = w / L::NSY, ys = v / NRAW, idx = v % NRAW;
+            const int w = it - 2 * NRAW * L::NSX, v = w / L::NSY;
             h = w % L::NSY; per = L::PERY;
-            fi = 10 + c_yt[idx];
-            ci = 9 + ys * 7 + c_yc[idx];
+            if (MIXED || v < NRAW) {
+                const int ys = v / NRAW, idx = v % NRAW;
+                fi = 10 + c_yt[idx];
+                ci = 9 + ys * 7 + c_yc[idx];
+            } else {                                                 // v = 0 row: M00, M01, M02 of the y- set from column 16
+                fi = 10 + (v - NRAW);
+                ci = 16;
+            }
             kb = 0; ke = NU;
         }
         const int b0 = min(kb + h * per, ke), b1 = min(kb + (h + 1) * per, ke);
@@ -172,6 +186,10 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
         o_first[q] = set < 2 ? v * L::NSX : 2 * NRAW * L::NSX + (v - 2 * NRAW) * L::NSY;
         if (!MIXED && set >= 2) set = ch.z > 0 ? 2 : 3;
         o_dst[q] = set * NRAW + idx;
+        if (!MIXED && v >= 3 * NRAW) {                               // the three y- outputs of the v = 0 row (flagged chunk only)
+            const int e = v - 3 * NRAW;
+            o_dst[q] = ch.w ? 3 * NRAW + (e == 0 ? RW_M00 : (e == 1 ? RW_M01 : RW_M02)) : -1;
+        }
     }
     __syncthreads();
 
@@ -207,6 +225,7 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
     }
     const bool ym_miss = beyond_wall_y(j - 1), yp_miss = beyond_wall_y(j + 1);
     const double sy = ch.z > 0 ? 1.0 : -1.0;                         // side of the y-contribution (uniform chunks)
+    const double wz = (ZROW && ch.w && r == 0 && active) ? 0.5 * c_wv[m0] : 0.0;
     // pipeline of one iteration a: stage 1 (cell a) -> [wait "part free"] store partials -> BARRIER -> (elected lane: bulk
     // copies of the freed slots) -> stage 2 (cell a) -> stage 3 (cell a - LAG3) -> stage 4 (cell a - LAG3 - 1)
     constexpr int LAG3 = R == 1 ? 0 : 1;
@@ -251,7 +270,8 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
                     // y-faces: n = v_m;  A_a = sum wv n^a f0 (a = 0..3),  B_a = sum wv n^a h sigma (a = 2..4)
                     if constexpr (!MIXED) {
                         const double f0 = fma(sy, hy, c);
-                        acc[6] = fma(w01.x, f0, acc[6]); acc[7] = fma(w01.y, f0, acc[7]); acc[8] = fma(w23.x, f0, acc[8]);
+                        if (ZROW && p == 0) acc[NA - 1] = wz * (c - hy);    // v = 0 row (row 0 of the flagged chunk): y- half
+                        acc[6] = fma(w4h.y, f0, acc[6]); acc[7] = fma(w01.y, f0, acc[7]); acc[8] = fma(w23.x, f0, acc[8]);
                         acc[9] = fma(w23.y, f0, acc[9]);
                         acc[10] = fma(w23.x, hy, acc[10]); acc[11] = fma(w23.y, hy, acc[11]); acc[12] = fma(w4h.x, hy, acc[12]);
                     } else {                                         // AMB-5: H(0) = 1/2 sends half of the point to either side
@@ -356,7 +376,7 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
 #pragma unroll
                     for (int h = 1; h < cmaxi(L::NSX, L::NSY); ++h)
                         if (h < ns) sum += ir[o_first[q] + h];
-                    dst[o_dst[q]] = sum;
+                    if (o_dst[q] >= 0) dst[o_dst[q]] = sum;
                 }
             }
         }

@@ -39,7 +39,9 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     constexpr int NY = SGN == 0 ? 4 : 3;
     using L = StageL<NY>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int c0 = s * STRIP, c1 = min(c0 + STRIP, GI);              // cells [c0, c1) of row j
+    // every CTA marches exactly STRIP cells (a compile-time trip count): the last strip of a row that STRIP does not divide
+    // starts at GI - STRIP and re-computes a few cells of its neighbour (same inputs, same arithmetic, same bits)
+    const int c0 = min(s * STRIP, GI - STRIP), c1 = c0 + STRIP;      // cells [c0, c1) of row j
     const int m0 = ch.x, mc = ch.y;
     const int q0 = m0 * NU, qa = q0 & ~1, qsh = q0 - qa;
     const uint32_t bytes = (uint32_t)(pad2c(mc * NU + qsh) * 8);

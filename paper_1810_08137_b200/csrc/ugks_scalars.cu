@@ -94,9 +94,10 @@ __device__ __forceinline__ void add_cell_raw(const UgksParams &P, int pos, int l
     const size_t cell = DIR == 0 ? (size_t)line * P.I + pos : (size_t)pos * P.I + line;
     const double *cm = P.cmom + cell * P.nchunk * CMS + set * NRAW;
     for (int c = 0; c < P.nchunk; ++c) {
-        const int sg = P.chunks[c].z;
+        const int4 ch = P.chunks[c];
+        const int sg = ch.z;
         if (set == 2 && sg < 0) continue;                            // a chunk of v < 0 rows holds no y+ part
-        if (set == 3 && sg > 0) continue;
+        if (set == 3 && sg > 0 && !ch.w) continue;                   // ... of v > 0 rows no y- part, unless it holds the v = 0 row
         for (int v = 0; v < NRAW; ++v) raw[v] += cm[c * CMS + v];
     }
 }

@@ -29,9 +29,8 @@ struct ugks_ctx {
     double kms[5]; long kcnt[5];
     // CUDA graph of two consecutive steps (launch-bound meshes): captured on an internal stream, replayed between two events
     int graph_mode;           // option "graph": -1 auto (on below 4e6 points per step), 0 off, 1 on
-    int graph_cur;            // parity of the state the graph starts from
-    long graph_launches;      // kernels inside the graph
-    cudaStream_t gst; cudaGraphExec_t gexec; cudaEvent_t gin, gout;
+    long graph_launches;      // kernels inside a graph
+    cudaStream_t gst; cudaGraphExec_t gexec[2]; cudaEvent_t gin, gout;       // gexec[p]: two steps starting from state parity p
     char err[256];
 };
 
@@ -484,7 +483,8 @@ int ugks_set_state(ugks_ctx *c, const double *W, const double *f, int on_dev)
 
 static void drop_graph(ugks_ctx *c)
 {
-    if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+    for (int p = 0; p < 2; ++p)
+        if (c->gexec[p]) { cudaGraphExecDestroy(c->gexec[p]); c->gexec[p] = nullptr; }
 }
 
 // one step of the five kernels on stream st, from state parity cur; returns the kernels launched
@@ -501,32 +501,42 @@ static long enqueue_step(ugks_ctx *c, int cur, cudaStream_t st)
     return n;
 }
 
-// replay pairs of steps from a captured graph; returns the steps done (0 if graphs are off or capture is not possible)
-static int step_by_graph(ugks_ctx *c, int n)
+// Launch-bound meshes replay pairs of steps from CUDA graphs captured on an internal stream.  Both graphs (one per parity of
+// the ping-pong state) are captured and instantiated by the FIRST ugks_step call of the context, however short, so that the
+// instantiation never falls into a later (timed) call and a call that starts from the other parity needs no re-capture.
+static bool graphs_wanted(const ugks_ctx *c)
 {
-    const bool want = c->graph_mode == 1 || (c->graph_mode < 0 && (double)c->cells * c->P.N < 4.0e6);
-    if (!want || c->profile || n < 4) return 0;
+    return !c->profile && (c->graph_mode == 1 || (c->graph_mode < 0 && (double)c->cells * c->P.N < 3.0e7));
+}
+static bool ensure_graphs(ugks_ctx *c)
+{
+    if (c->gexec[0] && c->gexec[1]) return true;
     if (!c->gst) {
         if (cudaStreamCreateWithFlags(&c->gst, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&c->gin, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&c->gout, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->graph_mode = 0; return 0; }
+            cudaEventCreateWithFlags(&c->gout, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); c->graph_mode = 0; return false; }
     }
-    if (c->gexec && c->graph_cur != c->cur) drop_graph(c);
-    if (!c->gexec) {
+    drop_graph(c);
+    for (int p = 0; p < 2; ++p) {
         cudaGraph_t g = nullptr;
-        if (cudaStreamBeginCapture(c->gst, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); c->graph_mode = 0; return 0; }
-        c->graph_launches = enqueue_step(c, c->cur, c->gst) + enqueue_step(c, c->cur ^ 1, c->gst);
-        if (cudaStreamEndCapture(c->gst, &g) != cudaSuccess || !g || cudaGraphInstantiate(&c->gexec, g, 0) != cudaSuccess) {
-            cudaGetLastError(); if (g) cudaGraphDestroy(g); c->gexec = nullptr; c->graph_mode = 0; return 0;
+        if (cudaStreamBeginCapture(c->gst, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); c->graph_mode = 0; return false; }
+        c->graph_launches = enqueue_step(c, p, c->gst) + enqueue_step(c, p ^ 1, c->gst);
+        if (cudaStreamEndCapture(c->gst, &g) != cudaSuccess || !g || cudaGraphInstantiate(&c->gexec[p], g, 0) != cudaSuccess) {
+            cudaGetLastError(); if (g) cudaGraphDestroy(g); c->gexec[p] = nullptr; drop_graph(c); c->graph_mode = 0; return false;
         }
         cudaGraphDestroy(g);
-        c->graph_cur = c->cur;
     }
+    return true;
+}
+// replay n / 2 pairs of steps; returns the steps done (0 if graphs are off or capture is not possible)
+static int step_by_graph(ugks_ctx *c, int n)
+{
+    if (!graphs_wanted(c) || !ensure_graphs(c) || n < 2) return 0;
     const int pairs = n / 2;
     if (cudaEventRecord(c->gin, c->st) != cudaSuccess || cudaStreamWaitEvent(c->gst, c->gin, 0) != cudaSuccess) { cudaGetLastError(); return 0; }
     int done = 0;
     for (int i = 0; i < pairs; ++i) {
-        if (cudaGraphLaunch(c->gexec, c->gst) != cudaSuccess) break;      // the error stays pending and surfaces in ugks_step
+        if (cudaGraphLaunch(c->gexec[c->cur], c->gst) != cudaSuccess) break;   // the error stays pending and surfaces in ugks_step
         ++done;
     }
     if (cudaEventRecord(c->gout, c->gst) == cudaSuccess) cudaStreamWaitEvent(c->st, c->gout, 0);

@@ -237,6 +237,10 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
 
     int xslot = 2 % NSXM, xphase = 2 / NSXM, ybuf_i = 0, yphase = 0; // ring slot / phase of row a+1 and of y stage a
     int issuer = 0;                                                  // lane 0 of a rotating warp issues the copies of a step
+#ifndef UGKS_UNROLL_M
+#define UGKS_UNROLL_M (STRIP >= 16 ? 2 : 1)                        // measured (C3, C4): -2 %; short strips: +10 %
+#endif
+#pragma unroll UGKS_UNROLL_M
     for (int a = c0; a < c1 + LAG3 + 1; ++a) {
         if (a < c1) {                                                // stage 1: point sums of cell a
             mbar_wait(&bars[xslot], xphase);                         // row a+1

@@ -75,6 +75,7 @@ def lib():
         L.ugkso_mu_ref.argtypes = [vp]; L.ugkso_mu_ref.restype = C.c_double
         L.ugkso_step_count.argtypes = [vp]; L.ugkso_step_count.restype = C.c_long
         L.ugkso_set_threads.argtypes = [vp, C.c_int]; L.ugkso_set_threads.restype = None
+        L.ugkso_set_tangential.argtypes = [vp, C.c_int]; L.ugkso_set_tangential.restype = None
         L.ugkso_destroy.argtypes = [vp]; L.ugkso_destroy.restype = None
         L.ugkso_face_flux.argtypes = [vp, C.c_int, C.c_int, C.c_int, _dp, _dp, _dp]
         L.ugkso_cell_update.argtypes = [vp, C.c_int, C.c_int, _dp, _dp]
@@ -156,7 +157,7 @@ class OracleError(RuntimeError):
 class Oracle:
     """One oracle context.  ``problem`` is a ``workloads.Problem``."""
 
-    def __init__(self, problem, threads: int | None = None):
+    def __init__(self, problem, threads: int | None = None, tangential: bool = False):
         L = lib()
         p = problem
         self.I, self.J, self.Nu, self.Nv = p.I, p.J, len(p.u), len(p.v)
@@ -173,6 +174,8 @@ class Oracle:
         self._h = h
         if threads:
             L.ugkso_set_threads(h, int(threads))
+        if tangential:
+            L.ugkso_set_tangential(h, 1)
 
     def _chk(self, rc, what):
         if rc:

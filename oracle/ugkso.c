@@ -169,6 +169,7 @@ struct ugkso_ctx {
     double *W, *Wn, *FWd;           /* W^n, W^{n+1}, accumulated macroscopic flux [J][I][4] */
     double res[4];
     long steps; int have_state, have_res, nthreads;
+    int tangential;                 /* O3t/O8t (NEXT-1): tangential slope theta of f in the free-transport part; default 0 */
 };
 
 enum { K_CELL = 0, K_GHOST = 1, K_WALL = 2 };
@@ -272,7 +273,7 @@ static void wall_face(const ugkso_ctx *c, int side, int ci, int cj, double FW[4]
     if (stage) { memset(stage, 0, 40 * sizeof(double)); stage[38] = rho_w; }
 }
 
-/* O2..O8: flux through one face.  scratch: 5*N doubles. */
+/* O2..O8: flux through one face.  scratch: 7*N doubles. */
 static int face_flux(const ugkso_ctx *c, int dir, int i, int j, double FW[4], double *Ff,
                      double *scratch, double *stage)
 {
@@ -286,8 +287,17 @@ static int face_flux(const ugkso_ctx *c, int dir, int i, int j, double FW[4], do
 
     double h = 0.5 * (dir == 0 ? c->dx : c->dy), ell = dir == 0 ? c->dy : c->dx, dt = c->dt;
     double *sigL = scratch, *sigR = scratch + N, *f0 = scratch + 2 * N, *s0 = scratch + 3 * N;
+    double *thL = scratch + 5 * N, *thR = scratch + 6 * N;          /* (scratch + 4N is used by wall_face) */
     cell_slope(c, dir, iL, jL, sigL);
     cell_slope(c, dir, iR, jR, sigR);
+    if (c->tangential) {
+        /* O3t (NEXT-1; "b (tangential)", ref [2]): the initial state is reconstructed in BOTH directions,
+         * f0(x,y) = f0 + sigma0 x + theta0 y on the upwind side, theta = the limited slope (O1) of the upwind cell in the
+         * TANGENTIAL direction.  At the face centre (y = 0) f0 and W0 are unchanged; free transport along the
+         * characteristic (x, y) = (-n t', -t t') adds -t t' theta0 under the time integral of Eq. (2). */
+        cell_slope(c, 1 - dir, iL, jL, thL);
+        cell_slope(c, 1 - dir, iR, jR, thR);
+    }
 
     /* O3 (S0/S1): upwind reconstruction at the face and its moments W0 */
     ksum W0s[4] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};
@@ -353,6 +363,8 @@ static int face_flux(const ugkso_ctx *c, int dir, int i, int j, double FW[4], do
         double e = 0.5 * (n * n + t * t);
         double g0 = ugkso_maxwellian(prim0, n, t);
         double r = Mt[3] * f0[q] - Mt[4] * n * s0[q];
+        if (c->tangential)                                                    /* O8t: ... - Mt5 t theta0, theta0 upwind */
+            r -= Mt[4] * t * (H * thL[q] + (1.0 - H) * thR[q]);
         ks_add(&Ffs[0], w * n * r);
         ks_add(&Ffs[1], w * n * n * r);
         ks_add(&Ffs[2], w * n * t * r);
@@ -471,6 +483,7 @@ int ugkso_init(ugkso_ctx **out, const ugkso_mesh *m, const ugkso_vgrid *vg, cons
 
 void ugkso_destroy(ugkso_ctx *c) { free_ctx(c); }
 void ugkso_set_threads(ugkso_ctx *c, int n) { if (c && n > 0) c->nthreads = n; }
+void ugkso_set_tangential(ugkso_ctx *c, int on) { if (c) c->tangential = on != 0; }
 double ugkso_dt(const ugkso_ctx *c) { return c ? c->dt : 0.0; }
 long ugkso_step_count(const ugkso_ctx *c) { return c ? c->steps : -1; }
 double ugkso_mu_ref(const ugkso_ctx *c) { return c ? c->mu_ref : 0.0; }
@@ -522,7 +535,7 @@ int ugkso_face_flux(ugkso_ctx *c, int dir, int i, int j, double FW[4], double *F
     if (!c->have_state) return UGKSO_ESTATE;
     if (dir == 0 && (i < 0 || i > c->I || j < 0 || j >= c->J)) return UGKSO_EINVAL;
     if (dir == 1 && (i < 0 || i >= c->I || j < 0 || j > c->J)) return UGKSO_EINVAL;
-    double *scratch = (double *)malloc(sizeof(double) * 5 * (size_t)c->N);
+    double *scratch = (double *)malloc(sizeof(double) * 7 * (size_t)c->N);
     if (!scratch) return UGKSO_ENOMEM;
     int rc = face_flux(c, dir, i, j, FW, Ff, scratch, stage);
     free(scratch);
@@ -535,7 +548,7 @@ int ugkso_cell_update(ugkso_ctx *c, int i, int j, double Wnew[4], double *fnew)
     if (!c || !Wnew || !fnew || i < 0 || i >= c->I || j < 0 || j >= c->J) return UGKSO_EINVAL;
     if (!c->have_state) return UGKSO_ESTATE;
     int N = c->N;
-    double *buf = (double *)malloc(sizeof(double) * 7 * (size_t)N);
+    double *buf = (double *)malloc(sizeof(double) * 9 * (size_t)N);
     if (!buf) return UGKSO_ENOMEM;
     double *Ff = buf, *Dq = buf + N, *scratch = buf + 2 * N, FW[4], FWd[4] = {0, 0, 0, 0};
     int rc = 0;
@@ -570,7 +583,7 @@ static int step_once(ugkso_ctx *c)
     /* x-faces: rows are independent (a face touches only cells of its row) */
     #pragma omp parallel num_threads(nth)
     {
-        double *buf = (double *)malloc(sizeof(double) * 6 * (size_t)N), FW[4];
+        double *buf = (double *)malloc(sizeof(double) * 8 * (size_t)N), FW[4];
         int lerr = buf ? 0 : UGKSO_ENOMEM;
         #pragma omp for schedule(static)
         for (int j = 0; j < J; ++j) {

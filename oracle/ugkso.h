@@ -54,6 +54,9 @@ double ugkso_dt(const ugkso_ctx *);
 long ugkso_step_count(const ugkso_ctx *);
 double ugkso_mu_ref(const ugkso_ctx *);
 void ugkso_set_threads(ugkso_ctx *, int nthreads);
+/* NEXT-1 (O3t/O8t): 1 = reconstruct f in the tangential direction too (limited slope theta of the upwind cell)
+ * and add -Mt5 t theta0 to the free-transport part of the face solution; default 0 (normal-direction reconstruction only). */
+void ugkso_set_tangential(ugkso_ctx *, int on);
 void ugkso_destroy(ugkso_ctx *);
 
 /* ---- one-by-one access (full-size sampled parity; stage-wise debugging) ---- */

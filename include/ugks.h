@@ -98,7 +98,9 @@ long ugks_launch_count(const ugks_ctx *);
  * are processed in parallel and a thread owns ceil(chunk / R) <= 16 points.  "strip", "chunk_m" (alias "chunk"), "R" set both
  * kernels; with the suffix "_u" (e.g. "R_u", "chunk_u") only k_flux_update, with "_m" ("R_m", "strip_m") only k_cell_moments.
  * The chunking of k_cell_moments may only coarsen its default (the moment buffer is sized for it).  Each change re-compiles
- * the kernel it touches.  Others: "profile" (1: time every kernel of ugks_step with CUDA events), "graph" (replay pairs of
+ * the kernel it touches.  "tangential" (O3t/O8t; default 0): 1 = f is reconstructed in the
+ * tangential direction of a face too (limited slope theta of the upwind cell) and the free-transport part of the face solution
+ * (Eq. (2)) carries -Mt5 t theta0; needs v-nodes that come in at most 8 runs of equal sign (ascending grids have 2); re-compiles both kernels.  Others: "profile" (1: time every kernel of ugks_step with CUDA events), "graph" (replay pairs of
  * steps from a CUDA graph: -1 auto = on for launch-bound meshes, 0 off, 1 on), "poison" (test aid: 1 = NaN-fill the shared
  * memory of every SM before each of the two f-sized kernels).
  * UGKS_EINVAL for unknown names or values that do not fit shared memory / the allocated buffers. */

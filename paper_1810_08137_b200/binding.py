@@ -109,7 +109,7 @@ class Ugks:
     ``ugks_mesh / ugks_vgrid / ugks_gas / ugks_bcs`` (see workloads.Problem).  Arrays passed to set_state / returned
     by f(), W() are torch CUDA tensors or numpy arrays; only their pointers cross the ABI."""
 
-    def __init__(self, problem, device="cuda:0", stream=None):
+    def __init__(self, problem, device="cuda:0", stream=None, tangential=False):
         import torch
         if not torch.cuda.is_available():
             raise UgksError(3, "no CUDA device: libugks has no CPU fallback")
@@ -131,6 +131,8 @@ class Ugks:
         if rc:
             raise UgksError(rc, L.ugks_last_error(None).decode())
         self._h = h
+        if tangential:
+            self.set_option("tangential", 1)
 
     def _chk(self, rc):
         if rc:

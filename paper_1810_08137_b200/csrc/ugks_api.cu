@@ -122,14 +122,33 @@ static void choose_R(int kind, int Nu, int cmax, int *R, int *npt)
     *R = best; *npt = (cmax + best - 1) / best;
 }
 
-static void choose_geometry(int kind, const double *v, int I, int J, int Nu, int Nv, KGeom *G)
+// the column ranges by sign of u (sorted nodes): a compile-time constant of k_cell_moments' stage 3
+static void set_u_ranges(UgksParams &T, const double *uhost)
 {
+    bool sorted = true;
+    for (int k = 1; k < T.Nu; ++k) if (uhost[k] < uhost[k - 1]) sorted = false;
+    T.kxm_end = T.Nu; T.kxp_begin = 0;
+    if (sorted) {
+        int k0 = 0, k1 = 0;
+        while (k0 < T.Nu && uhost[k0] < 0.0) ++k0;                   // first u >= 0
+        k1 = k0; while (k1 < T.Nu && uhost[k1] <= 0.0) ++k1;         // first u > 0
+        T.kxp_begin = k0; T.kxm_end = k1;
+    }
+    T.s3_nsx = T.s3_nsy = 0;                                         // (the stage-3 split is a compile-time constant of the kernel)
+}
+// default launch geometry of kernel `kind` for the sizes, node signs and options (tangential) in T: the largest chunk of at
+// most the target rows whose CTA fits the 227 KB of shared memory
+static void choose_geometry(int kind, const UgksParams &T, const double *v, KGeom *G)
+{
+    const int Nu = T.Nu;
     int cm = 800 / Nu; if (cm < 1) cm = 1; if (cm > 56) cm = 56;
     if (Nu > 128) cm = kind == JIT_MOMENTS ? 14 : 5;                 // wide rows: one thread per column (measured, C5)
-    make_chunks(v, Nv, Nu, cm, G);
-    choose_R(kind, Nu, G->cmax, &G->R, &G->npt);
+    for (; cm >= 1; --cm) {
+        make_chunks(v, T.Nv, Nu, cm, G);
+        choose_R(kind, Nu, G->cmax, &G->R, &G->npt);
+        if (jit_smem(kind, T, *G) <= 227 * 1024) break;
+    }
     G->strip = 0;                                                    // 0 = automatic (default_strip / choose_strip in apply_geometry)
-    (void)I; (void)J;
 }
 
 static int default_strip(int I) { const int ns = (I + 31) / 32; return (I + ns - 1) / ns; }     // balanced strips of <= 32 cells
@@ -169,9 +188,17 @@ static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
     L->frs = FR_NCOEF + L->NuP + L->NvP; L->crs = CR_NCOEF + 2 * L->NuP + 2 * L->NvP;
     // the moment buffer holds the chunks of the default geometry (the "chunk_m" tuning option may only coarsen it)
     if (!vg->v) return 1;
-    KGeom G;
-    choose_geometry(JIT_MOMENTS, vg->v, m->I, m->J, vg->Nu, vg->Nv, &G);
-    size_t nchunk = (size_t)G.nchunk();
+    if (!vg->u) return 1;
+    size_t nchunk = 0;
+    for (int tg = 0; tg < 2; ++tg) {                                 // room for the chunking with and without option "tangential"
+        UgksParams T;
+        memset(&T, 0, sizeof T);
+        T.I = m->I; T.J = m->J; T.Nu = vg->Nu; T.Nv = vg->Nv; T.NuP = L->NuP; T.NvP = L->NvP; T.frs = L->frs; T.crs = L->crs; T.tangential = tg;
+        set_u_ranges(T, vg->u);
+        KGeom G;
+        choose_geometry(JIT_MOMENTS, T, vg->v, &G);
+        if ((size_t)G.nchunk() > nchunk) nchunk = (size_t)G.nchunk();
+    }
     if (nchunk < 1 || nchunk > MAXCHUNK) return 1;
     L->nchunk_alloc = (int)nchunk;
     L->Npad = (int)Npad;
@@ -196,20 +223,6 @@ static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
     return 0;
 }
 
-// the column ranges by sign of u (sorted nodes): a compile-time constant of k_cell_moments' stage 3
-static void set_u_ranges(UgksParams &T, const double *uhost)
-{
-    bool sorted = true;
-    for (int k = 1; k < T.Nu; ++k) if (uhost[k] < uhost[k - 1]) sorted = false;
-    T.kxm_end = T.Nu; T.kxp_begin = 0;
-    if (sorted) {
-        int k0 = 0, k1 = 0;
-        while (k0 < T.Nu && uhost[k0] < 0.0) ++k0;                   // first u >= 0
-        k1 = k0; while (k1 < T.Nu && uhost[k1] <= 0.0) ++k1;         // first u > 0
-        T.kxp_begin = k0; T.kxm_end = k1;
-    }
-    T.s3_nsx = T.s3_nsy = 0;                                         // (the stage-3 split is a compile-time constant of the kernel)
-}
 // is G a launchable geometry of kernel `kind`?  returns a message if not
 static const char *check_geometry(int kind, const UgksParams &T, const KGeom &G)
 {
@@ -276,10 +289,11 @@ int ugks_jit_check(const ugks_mesh *m, const ugks_vgrid *vg, const ugks_bcs *bcs
     const ugks_bc *b[4] = { &bcs->xmin, &bcs->xmax, &bcs->ymin, &bcs->ymax };
     for (int s = 0; s < 4; ++s) T.bc[s] = b[s]->type;
     set_u_ranges(T, vg->u);
+    if (const char *e = getenv("UGKS_JIT_CHECK_TANGENTIAL")) T.tangential = atoi(e) != 0;      // developer aid: check the TG variants
     std::string all;
     for (int kind = 0; kind < 2; ++kind) {
         KGeom G;
-        choose_geometry(kind, vg->v, T.I, T.J, T.Nu, T.Nv, &G);
+        choose_geometry(kind, T, vg->v, &G);
         G.strip = default_strip(T.I);
         if (const char *why = check_geometry(kind, T, G)) return fail(nullptr, UGKS_EINVAL, "%s", why);
         std::vector<char> cubin;
@@ -371,7 +385,7 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     set_u_ranges(P, c->uhost);
     c->gm = new KGeom(); c->gu = new KGeom();
     KGeom G0[2];
-    for (int kind = 0; kind < 2; ++kind) choose_geometry(kind, vg->v, P.I, P.J, P.Nu, P.Nv, &G0[kind]);
+    for (int kind = 0; kind < 2; ++kind) choose_geometry(kind, P, vg->v, &G0[kind]);
     if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c->gm; delete c->gu; free(c->vhost); free(c); return fail(nullptr, UGKS_ECUDA, "%s", "cudaGetDevice failed"); }
 
     double bcprim[16];
@@ -449,6 +463,18 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
             }
             return UGKS_OK;
         }
+    }
+    if (!strcmp(name, "tangential")) {                               // NEXT-1 (O3t/O8t): re-compiles both kernels
+        if (c->gm->nmix > 0 || c->gu->nmix > 0) return fail(c, UGKS_EINVAL, "%s", "the tangential reconstruction needs v-nodes in runs of equal sign (no mixed-sign chunks)");
+        const int old = P.tangential;
+        P.tangential = value != 0;
+        for (int kind = 0; kind < 2; ++kind) {                       // default geometry of the new mode (the staged rows differ)
+            KGeom G;
+            choose_geometry(kind, P, c->vhost, &G);
+            const int rc = apply_geometry(c, kind, G);
+            if (rc) { P.tangential = old; return rc; }
+        }
+        return UGKS_OK;
     }
     if (!strcmp(name, "profile")) { c->profile = value != 0; return UGKS_OK; }
     if (!strcmp(name, "poison")) { c->poison = value != 0; drop_graph(c); return UGKS_OK; }

@@ -14,8 +14,11 @@ enum { BC_PERIODIC = 0, BC_FIXED = 1, BC_WALL = 2 };
 // A cell contributes (f_c + h sigma_c) to its plus-side face where n > 0 and (f_c - h sigma_c) to its minus-side face
 // where n < 0 (O3 written cell by cell); sets: 0 = x+, 1 = x-, 2 = y+, 3 = y-.  13 raw sums per set, local frame,
 // M_ab = sum w n^a t^b f0, S_ab = sum w n^a t^b (h sigma0):
-constexpr int NSET = 4, NRAW = 13, CMS = NSET * NRAW;
-enum { RW_M00 = 0, RW_M10, RW_M20, RW_M30, RW_M01, RW_M11, RW_M02, RW_M12, RW_S20, RW_S30, RW_S40, RW_S21, RW_S22 };
+// With the tangential reconstruction of f (option "tangential", O3t/O8t) five more, T_ab = sum w n^a t^b (h_t theta0), h_t = half
+// the tangential spacing; the storage always has room for them.
+constexpr int NSET = 4, NRAW = 18, NRAW_BASE = 13, CMS = NSET * NRAW;
+enum { RW_M00 = 0, RW_M10, RW_M20, RW_M30, RW_M01, RW_M11, RW_M02, RW_M12, RW_S20, RW_S30, RW_S40, RW_S21, RW_S22,
+       RW_T11, RW_T21, RW_T12, RW_T31, RW_T13 };
 
 // Face record written by k_face_scalars (S2..S5; 24 coefficients) and k_tables (separable Maxwellian factors):
 //   [0, FR_NCOEF)                        coefficients, see FR_*
@@ -25,7 +28,8 @@ enum { RW_M00 = 0, RW_M10, RW_M20, RW_M30, RW_M01, RW_M11, RW_M02, RW_M12, RW_S2
 // coefficients that contain a (c10, c20, c30, c11, c12) come in an L (n > 0, a_L) and an R (n < 0, a_R) variant.
 constexpr int FR_NCOEF = 24;
 enum { FR_LAM = 0, FR_U = 1, FR_V = 2, FR_TYPE = 3, FR_RHOW = 4, FR_MT4 = 5 /* ell Mt4 */, FR_MT5 = 6 /* -ell Mt5 2/Delta */,
-       FR_TAU = 7, FR_C00 = 8, FR_C01 = 9, FR_C02 = 10, FR_C03 = 11, FR_C21 = 12, FR_L = 13, FR_R = 18 };
+       FR_TAU = 7, FR_C00 = 8, FR_C01 = 9, FR_C02 = 10, FR_C03 = 11, FR_C21 = 12, FR_L = 13, FR_R = 18,
+       FR_MT5T = 23 /* -ell Mt5 2/Delta_t (tangential spacing); 0 unless option "tangential" */ };
 // offsets inside FR_L / FR_R
 enum { LR_C10 = 0, LR_C20 = 1, LR_C30 = 2, LR_C11 = 3, LR_C12 = 4 };
 
@@ -43,6 +47,7 @@ struct UgksParams {
     int frs, crs;                    // record strides in doubles: FR_NCOEF + NuP + NvP, CR_NCOEF + 2 NuP + 2 NvP
     double dx, dy, dt, omega, mu_ref;
     int bc[4];                       // xmin, xmax, ymin, ymax
+    int tangential;                  // option "tangential" (NEXT-1, O3t/O8t): f is reconstructed in the tangential direction too
     const double *u, *wu, *v, *wv;   // device copies of the velocity nodes / weights
     const double *ghost;             // [4][Npad] FIXED ghost rows f_b (O0)
     const double *wallg;             // [4][Npad] wall Maxwellians of (1,Uw,Vw,1/Tw) (O0)

@@ -35,12 +35,13 @@ int smem_mom(const UgksParams &P, const KGeom &G, bool mixed)
     const int BT = (P.Nu * G.R + 31) / 32 * 32, QB = pad2i(G.cmax * P.Nu + 1);
     bool zrow = false;
     for (const int4 &c : G.chunks) if (c.w) zrow = true;
-    const int NA = mixed ? 20 : (zrow ? 14 : 13), NC = mixed ? 23 : (zrow ? 17 : 16), ny = mixed ? 26 : (zrow ? 16 : 13);
+    const int nrk = P.tangential ? 18 : 13;
+    const int NA = mixed ? 20 : 13 + (P.tangential ? 6 : 0) + (zrow ? 1 : 0), NC = NA + 3, ny = mixed ? 2 * nrk : nrk + (zrow ? 3 : 0);
     const int lenx = P.kxm_end > P.Nu - P.kxp_begin ? P.kxm_end : P.Nu - P.kxp_begin;
     int per = P.Nu;
-    for (int q = 1; q <= P.Nu; ++q) if (26 * cdivi(lenx, q) + ny * cdivi(P.Nu, q) <= BT) { per = q; break; }
-    const int nitem = 26 * cdivi(lenx, per) + ny * cdivi(P.Nu, per), NUS = P.Nu | 1, NROW = G.R * G.npt + 1;
-    const int total = nsxm() * QB + 4 * QB + (G.R == 1 ? 0 : NA * BT) + pad2i(2 * NC * NUS) + pad2i(13 * NUS) + pad2i(NROW * 6) +
+    for (int q = 1; q <= P.Nu; ++q) if (2 * nrk * cdivi(lenx, q) + ny * cdivi(P.Nu, q) <= BT) { per = q; break; }
+    const int nitem = 2 * nrk * cdivi(lenx, per) + ny * cdivi(P.Nu, per), NUS = P.Nu | 1, NROW = G.R * G.npt + 1;
+    const int total = nsxm() * QB + 4 * QB + (G.R == 1 ? 0 : NA * BT) + pad2i(2 * NC * NUS) + pad2i(14 * NUS) + pad2i(NROW * 6) +
                       pad2i(2 * nitem) + nsxm() + 3;
     return total * 8;
 }
@@ -97,7 +98,7 @@ void add_doubles(std::string &s, const char *name, const double *a, int n)
 size_t jit_smem(int kind, const UgksParams &P, const KGeom &G)
 {
     if (kind == JIT_MOMENTS) return (size_t)smem_mom(P, G, G.nmix > 0);
-    return (size_t)smem_upd(P, G, G.nmix > 0 ? 4 : 3);
+    return (size_t)smem_upd(P, G, G.nmix > 0 ? 4 : (P.tangential ? 6 : 3));
 }
 
 std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const double *u, const double *wu, const double *v, const double *wv)
@@ -111,13 +112,14 @@ std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const dou
     DEF("G_BC0", P.bc[0]); DEF("G_BC1", P.bc[1]); DEF("G_BC2", P.bc[2]); DEF("G_BC3", P.bc[3]);
     DEF("G_NCHUNK", G.nchunk()); DEF("G_NMIX", G.nmix); DEF("G_MC", G.cmax); DEF("G_R", G.R); DEF("G_NPT", G.npt); DEF("G_STRIP", G.strip);
     { int z = 0; for (const int4 &c : G.chunks) if (c.w) z = 1; DEF("G_HAS_ZROW", z); }
+    DEF("G_TANGENTIAL", P.tangential ? 1 : 0);
     DEF("G_KXM_END", P.kxm_end); DEF("G_KXP_BEGIN", P.kxp_begin); DEF("G_RAGGED", G.ragged() ? 1 : 0);
     if (kind == JIT_MOMENTS) {
         const int sm_u = smem_mom(P, G, false), sm_m = smem_mom(P, G, true);
         DEF("G_SMEM_MOM", sm_u); DEF("G_SMEM_MOMX", sm_m); DEF("G_NSXM", nsxm());
         DEF("G_MINB_MOM", min_blocks(threads, sm_u, 128)); DEF("G_MINB_MOMX", min_blocks(threads, sm_m, 128));
     } else {
-        const int su3 = smem_upd(P, G, 3), su4 = smem_upd(P, G, 4);
+        const int su3 = smem_upd(P, G, P.tangential ? 6 : 3), su4 = smem_upd(P, G, 4);
         DEF("G_SMEM_UPD3", su3); DEF("G_SMEM_UPD4", su4);
         DEF("G_MINB_UPD", min_blocks(threads, G.nmix > 0 ? su4 : su3, 128));
     }
@@ -180,7 +182,7 @@ int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, cons
         if (e != cudaSuccess) { snprintf(err, errlen, "JIT load failed: %s", cudaGetErrorString(e)); delete m; return 1; }
         m->threads = threads_of(kind, P, G);
         if (kind == JIT_MOMENTS) { m->smem = smem_mom(P, G, false); m->smemx = smem_mom(P, G, true); }
-        else m->smem = smem_upd(P, G, G.nmix > 0 ? 4 : 3);
+        else m->smem = smem_upd(P, G, G.nmix > 0 ? 4 : (P.tangential ? 6 : 3));
         g_cache[key] = m;
     }
     // shared-memory opt-in: a function attribute of the CURRENT device, set for every context (cheap, idempotent)

@@ -33,12 +33,15 @@ constexpr int QB = pad2c(MC * NU + 1);                                // doubles
 constexpr int QBB = QB * 8;
 
 // per-(cell, chunk) half-range raw moment sets (see ugks_common.cuh): sets 0 = x+, 1 = x-, 2 = y+, 3 = y-
-constexpr int NSET = 4, NRAW = 13, CMS = NSET * NRAW;
-enum { RW_M00 = 0, RW_M10, RW_M20, RW_M30, RW_M01, RW_M11, RW_M02, RW_M12, RW_S20, RW_S30, RW_S40, RW_S21, RW_S22 };
+// TG: option "tangential" (NEXT-1, O3t/O8t): five more raw sums per set, T_ab = sum w n^a t^b (h_t theta0)
+constexpr bool TG = G_TANGENTIAL != 0;
+constexpr int NSET = 4, NRAW = 18, NRK = TG ? 18 : 13, CMS = NSET * NRAW;       // storage stride / sums a kernel computes
+enum { RW_M00 = 0, RW_M10, RW_M20, RW_M30, RW_M01, RW_M11, RW_M02, RW_M12, RW_S20, RW_S30, RW_S40, RW_S21, RW_S22,
+       RW_T11, RW_T21, RW_T12, RW_T31, RW_T13 };
 // face / cell record layout (see ugks_common.cuh)
 constexpr int FR_NCOEF = 24;
 enum { FR_LAM = 0, FR_U = 1, FR_V = 2, FR_TYPE = 3, FR_RHOW = 4, FR_MT4 = 5, FR_MT5 = 6, FR_TAU = 7, FR_C00 = 8, FR_C01 = 9,
-       FR_C02 = 10, FR_C03 = 11, FR_C21 = 12, FR_L = 13, FR_R = 18 };
+       FR_C02 = 10, FR_C03 = 11, FR_C21 = 12, FR_L = 13, FR_R = 18, FR_MT5T = 23 };
 enum { LR_C10 = 0, LR_C20 = 1, LR_C30 = 2, LR_C11 = 3, LR_C12 = 4 };
 constexpr int CR_NCOEF = 12;
 enum { CR_KF = 0, CR_KD = 1 };
@@ -84,6 +87,30 @@ __device__ __forceinline__ const double *yrow_base(const double *f, const double
         else pos = GJ - 1;
     }
     return f + (size_t)pos * GI * NPAD;
+}
+// row of cell (i, jj) with BOTH directions resolved the way the neighbour lookup of O1 does (x first): PERIODIC wraps, a FIXED
+// side returns its ghost row, a WALL neighbour is "missing" (a clamped valid row whose values are never used)
+__device__ __forceinline__ const double *cell_row_ptr(const double *f, const double *ghost, int i, int jj)
+{
+    if (i < 0) {
+        if (BCX0 == BC_PERIODIC) i += GI;
+        else if (BCX0 == BC_FIXED) return ghost;
+        else i = 0;
+    } else if (i >= GI) {
+        if (BCX1 == BC_PERIODIC) i -= GI;
+        else if (BCX1 == BC_FIXED) return ghost + NPAD;
+        else i = GI - 1;
+    }
+    if (jj < 0) {
+        if (BCY0 == BC_PERIODIC) jj += GJ;
+        else if (BCY0 == BC_FIXED) return ghost + 2 * NPAD;
+        else jj = 0;
+    } else if (jj >= GJ) {
+        if (BCY1 == BC_PERIODIC) jj -= GJ;
+        else if (BCY1 == BC_FIXED) return ghost + 3 * NPAD;
+        else jj = GJ - 1;
+    }
+    return f + ((size_t)jj * GI + i) * NPAD;
 }
 __device__ __forceinline__ bool beyond_wall_x(int pos) { return (pos < 0 && BCX0 == BC_WALL) || (pos >= GI && BCX1 == BC_WALL); }
 __device__ __forceinline__ bool beyond_wall_y(int pos) { return (pos < 0 && BCY0 == BC_WALL) || (pos >= GJ && BCY1 == BC_WALL); }

@@ -23,12 +23,14 @@
 
 constexpr int NSXM = G_NSXM;                                         // x-ring slots (>= 2)
 constexpr int NW = BT / 32;                                          // warps of a CTA
-constexpr int NFAC = 13;                                             // factor tables: 5 (x+), 5 (x-), 3 (y)
-// raw sum idx -> (power of the per-column velocity, column sum) ; x sets: columns 0..2 = C_b +- B_b, 3..5 = B_b
-__constant__ int c_xa[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 2, 3, 4, 2, 2 };
-__constant__ int c_xc[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 3, 3, 3, 4, 5 };
-__constant__ int c_yt[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 0, 0, 0, 1, 2 };   // y sets: columns A_0..A_3, B_2..B_4
-__constant__ int c_yc[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 4, 5, 6, 4, 4 };
+constexpr int NFAC = 14;                                             // factor tables: 5 (x+), 5 (x-), 4 (y)
+// raw sum idx -> (power of the per-column velocity, column sum) ; x sets: columns 0..2 = C_b +- B_b, 3..5 = B_b, and with TG
+// 6..8 = D_1..D_3 = sum wv v^b (h_y sigma_y) (the tangential slope on an x-face is the cell's y-slope)
+__constant__ int c_xa[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 2, 3, 4, 2, 2,   1, 2, 1, 3, 1 };
+__constant__ int c_xc[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 3, 3, 3, 4, 5,   6, 6, 7, 6, 8 };
+// y sets: columns A_0..A_3, B_2..B_4, and with TG E_1..E_3 = sum wv v^a (h_x sigma_x) (columns 10..12)
+__constant__ int c_yt[NRAW] = { 0, 0, 0, 0, 1, 1, 2, 2, 0, 0, 0, 1, 2,   1, 1, 2, 1, 3 };
+__constant__ int c_yc[NRAW] = { 0, 1, 2, 3, 0, 1, 0, 1, 4, 5, 6, 4, 4,   10, 11, 10, 12, 10 };
 
 constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
 constexpr int cmaxi(int a, int b) { return a > b ? a : b; }
@@ -41,23 +43,24 @@ constexpr bool ZROW = G_HAS_ZROW != 0;
 constexpr int NYX = ZROW ? 3 : 0;                                    // extra y- outputs of the chunk that holds the v = 0 row
 constexpr int s3_per(bool mixed)
 {
-    const int lenx = cmaxi(KXM_END, NU - KXP_BEGIN), ny = mixed ? 2 * NRAW : NRAW + NYX;
+    const int lenx = cmaxi(KXM_END, NU - KXP_BEGIN), ny = mixed ? 2 * NRK : NRK + NYX;
     for (int per = 1; per <= NU; ++per)
-        if (2 * NRAW * cdiv(lenx, per) + ny * cdiv(NU, per) <= BT) return per;
+        if (2 * NRK * cdiv(lenx, per) + ny * cdiv(NU, per) <= BT) return per;
     return NU;
 }
 
 template <bool MIXED>
 struct MomL {                                                        // sizes and the shared-memory carve-up (offsets in doubles)
-    static constexpr int NA = MIXED ? 20 : (ZROW ? 14 : 13);         // per-thread sums: 6 (x) + 7 (y) [+ 7 (y-) | + 1 (v = 0 row)]
-    static constexpr int NC = MIXED ? 23 : (ZROW ? 17 : 16);         // columns after stage 2: 9 (x) + 7 (y) [+ 7 | + 1]
-    static constexpr int NYO = MIXED ? 2 * NRAW : NRAW + NYX;        // y outputs of a chunk
-    static constexpr int NOUT = 2 * NRAW + NYO;
+    static constexpr int NTG = TG ? 6 : 0;                           // D_1..D_3, E_1..E_3
+    static constexpr int NA = MIXED ? 20 : 13 + NTG + (ZROW ? 1 : 0);   // per-thread sums: 6 (x) + 7 (y) [+ 7 (y-) | + 6 (TG) + 1 (v = 0 row)]
+    static constexpr int NC = NA + 3;                                // columns after stage 2: 9 (x) + (NA - 6)
+    static constexpr int NYO = MIXED ? 2 * NRK : NRK + NYX;          // y outputs of a chunk
+    static constexpr int NOUT = 2 * NRK + NYO;
     static constexpr int LENX = cmaxi(KXM_END, NU - KXP_BEGIN);
     static constexpr int PER = s3_per(MIXED);
     static constexpr int NSX = cdiv(LENX, PER), NSY = cdiv(NU, PER);
     static constexpr int PERX = cdiv(LENX, NSX), PERY = cdiv(NU, NSY);
-    static constexpr int NITEM = 2 * NRAW * NSX + NYO * NSY;
+    static constexpr int NITEM = 2 * NRK * NSX + NYO * NSY;
     static constexpr int NUS = NU | 1;                               // odd column stride
     static constexpr int NROW = R * NPT + 1;                         // weight rows incl. zero rows for a ragged chunk
     static constexpr int O_YBUF = NSXM * QB;
@@ -134,7 +137,7 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
         for (int a = 0; a < 5; ++a) {
             fac[a * NUS + i] = w * hp * pw;
             fac[(5 + a) * NUS + i] = w * (1.0 - hp) * pw;
-            if (a < 3) fac[(10 + a) * NUS + i] = w * pw;
+            if (a < 4) fac[(10 + a) * NUS + i] = w * pw;
             pw *= u;
         }
     }
@@ -153,22 +156,22 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
     for (int q = 0; q < S3R; ++q) {
         const int it = tid + q * BT;
         int fi = 0, ci = 0, kb = 0, ke = 0, h = 0, per = 1;
-        if (it < 2 * NRAW * L::NSX) {
-            const int v = it / L::NSX, set = v / NRAW, idx = v % NRAW, c = c_xc[idx];
+        if (it < 2 * NRK * L::NSX) {
+            const int v = it / L::NSX, set = v / NRK, idx = v % NRK, c = c_xc[idx];
             h = it % L::NSX; per = L::PERX;
             fi = (set == 0 ? 0 : 5) + c_xa[idx];
-            ci = c < 3 ? (set == 0 ? c : 3 + c) : 3 + c;             // columns: 0..2 C+B, 3..5 C-B, 6..8 B
+            ci = c < 3 ? (set == 0 ? c : 3 + c) : (c < 6 ? 3 + c : 10 + c);   // columns: 0..2 C+B, 3..5 C-B, 6..8 B, 16..18 D (TG)
             kb = set == 0 ? KXP_BEGIN : 0; ke = set == 0 ? NU : KXM_END;
         } else if (it < NITEM) {
-            const int w = it - 2 * NRAW * L::NSX, v = w / L::NSY;
+            const int w = it - 2 * NRK * L::NSX, v = w / L::NSY;
             h = w % L::NSY; per = L::PERY;
-            if (MIXED || v < NRAW) {
-                const int ys = v / NRAW, idx = v % NRAW;
+            if (MIXED || v < NRK) {
+                const int ys = v / NRK, idx = v % NRK;
                 fi = 10 + c_yt[idx];
                 ci = 9 + ys * 7 + c_yc[idx];
-            } else {                                                 // v = 0 row: M00, M01, M02 of the y- set from column 16
-                fi = 10 + (v - NRAW);
-                ci = 16;
+            } else {                                                 // v = 0 row: M00, M01, M02 of the y- set from the last column
+                fi = 10 + (v - NRK);
+                ci = NC - 1;
             }
             kb = 0; ke = NU;
         }
@@ -181,13 +184,13 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
 #pragma unroll
     for (int q = 0; q < S4R; ++q) {
         const int v = tid + q * BT;
-        int set = v / NRAW;
-        const int idx = v % NRAW;
-        o_first[q] = set < 2 ? v * L::NSX : 2 * NRAW * L::NSX + (v - 2 * NRAW) * L::NSY;
+        int set = v / NRK;
+        const int idx = v % NRK;
+        o_first[q] = set < 2 ? v * L::NSX : 2 * NRK * L::NSX + (v - 2 * NRK) * L::NSY;
         if (!MIXED && set >= 2) set = ch.z > 0 ? 2 : 3;
         o_dst[q] = set * NRAW + idx;
-        if (!MIXED && v >= 3 * NRAW) {                               // the three y- outputs of the v = 0 row (flagged chunk only)
-            const int e = v - 3 * NRAW;
+        if (!MIXED && v >= 3 * NRK) {                                // the three y- outputs of the v = 0 row (flagged chunk only)
+            const int e = v - 3 * NRK;
             o_dst[q] = ch.w ? 3 * NRAW + (e == 0 ? RW_M00 : (e == 1 ? RW_M01 : RW_M02)) : -1;
         }
     }
@@ -278,6 +281,10 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
                         acc[6] = fma(w4h.y, f0, acc[6]); acc[7] = fma(w01.y, f0, acc[7]); acc[8] = fma(w23.x, f0, acc[8]);
                         acc[9] = fma(w23.y, f0, acc[9]);
                         acc[10] = fma(w23.x, hy, acc[10]); acc[11] = fma(w23.y, hy, acc[11]); acc[12] = fma(w4h.x, hy, acc[12]);
+                        if constexpr (TG) {                          // tangential slopes: D_b = sum wv v^b (h_y sigma_y), E_a = sum wv v^a (h_x sigma_x)
+                            acc[13] = fma(w01.y, hy, acc[13]); acc[14] = fma(w23.x, hy, acc[14]); acc[15] = fma(w23.y, hy, acc[15]);
+                            acc[16] = fma(w01.y, hx, acc[16]); acc[17] = fma(w23.x, hx, acc[17]); acc[18] = fma(w23.y, hx, acc[18]);
+                        }
                     } else {                                         // AMB-5: H(0) = 1/2 sends half of the point to either side
                         const double hp = w4h.y, hm = 1.0 - hp, fp = (c + hy) * hp, fm = (c - hy) * hm, gp = hy * hp, gm = hy * hm;
                         acc[6] = fma(w01.x, fp, acc[6]); acc[7] = fma(w01.y, fp, acc[7]); acc[8] = fma(w23.x, fp, acc[8]);
@@ -375,7 +382,7 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
             for (int q = 0; q < S4R; ++q) {
                 const int v = tid + q * BT;
                 if (v < NOUT) {
-                    const int ns = v < 2 * NRAW ? L::NSX : L::NSY;
+                    const int ns = v < 2 * NRK ? L::NSX : L::NSY;
                     double sum = ir[o_first[q]];
 #pragma unroll
                     for (int h = 1; h < cmaxi(L::NSX, L::NSY); ++h)
@@ -387,7 +394,11 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
     }
 }
 
-static_assert(MomL<false>::BYTES == G_SMEM_MOM && MomL<true>::BYTES == G_SMEM_MOMX, "host mirror of the shared-memory layout (ugks_jit.cu) disagrees");
+static_assert(MomL<false>::BYTES == G_SMEM_MOM, "host mirror of the shared-memory layout (ugks_jit.cu) disagrees");
+#if G_NMIX > 0
+static_assert(MomL<true>::BYTES == G_SMEM_MOMX, "host mirror of the shared-memory layout (ugks_jit.cu) disagrees");
+static_assert(!TG, "the tangential reconstruction needs sorted velocity nodes (no mixed-sign chunks)");
+#endif
 
 #ifdef UGKS_MINB_MOM                                                // experiment override (UGKS_JIT_DEFS)
 #undef G_MINB_MOM

@@ -14,6 +14,10 @@
 //   * y-stencil: three rows ((j-2, j-1, j+1) for v > 0, (j-1, j+1, j+2) for v < 0) are TMA-staged per cell, double-buffered,
 //     together with the records of the step (face and cell coefficients, separable factors; whole records, one copy each).
 //   * f^{n+1} is written straight from registers: f crosses HBM once each way in this kernel.
+//   * option "tangential" (TG; NEXT-1, O3t/O8t): every face flux gets -ell Mt5 n t theta0, theta0 = the limited slope of the upwind
+//     cell in the face's tangential direction.  Three more rows are staged per step -- the x-neighbours (c-1, jn), (c+1, jn) of
+//     the upwind y-neighbour row jn and (c+1, jo) on the other side -- so that every slope is formed from explicitly staged rows;
+//     the x-slope of the own cell is the x-face limiter result of this step (u > 0) or of the previous one (u < 0).
 //   * there is no producer warp: after the barrier that ends step a, one lane of warp (a mod W) issues the 8 bulk copies of
 //     step a+2 / row a+3 (with compile-time geometry that is a few dozen instructions), so every resident warp computes and
 //     no warp's registers idle.
@@ -36,7 +40,7 @@ struct StageL {                                                      // offsets 
 template <int SGN>
 __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, const int j, const int s)
 {
-    constexpr int NY = SGN == 0 ? 4 : 3;
+    constexpr int NY = SGN == 0 ? 4 : (TG ? 6 : 3);
     using L = StageL<NY>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     // every CTA marches exactly STRIP cells (a compile-time trip count): the last strip of a row that STRIP does not divide
@@ -69,6 +73,27 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         double *S = stages + sl * L::size;
         uint64_t *bar = &bars[NSX + sl];
         const bool have_cell = st > c0;
+        if constexpr (TG) {
+            // rows relative to c = st - 1 (also for st = c0: x-face c0 needs the y-slope of its upwind cell c0-1 or c0):
+            // 0..2 as without TG; 3 = (c-1, jn), 4 = (c+1, jn), 5 = (c+1, jo) with jn the upwind y-neighbour row of the chunk's sign
+            constexpr int JN = SGN > 0 ? -1 : 1, JO = -JN;
+            const int c = st - 1;
+            mbar_expect_tx(bar, fbytes + 6 * bytes + (have_cell ? 2 * fbytes + cbytes : 0));
+            tma_load_1d(S + L::xrec, A.frec0 + ((size_t)j * (GI + 1) + st) * FRS, fbytes, bar);
+            tma_load_1d(S + L::yrow, cell_row_ptr(fcur, A.ghost, c, j + DJ0) + qa, bytes, bar);
+            tma_load_1d(S + L::yrow + QB, cell_row_ptr(fcur, A.ghost, c, j + DJ1) + qa, bytes, bar);
+            tma_load_1d(S + L::yrow + 2 * QB, cell_row_ptr(fcur, A.ghost, c, j + DJ2) + qa, bytes, bar);
+            tma_load_1d(S + L::yrow + 3 * QB, cell_row_ptr(fcur, A.ghost, c - 1, j + JN) + qa, bytes, bar);
+            tma_load_1d(S + L::yrow + 4 * QB, cell_row_ptr(fcur, A.ghost, c + 1, j + JN) + qa, bytes, bar);
+            tma_load_1d(S + L::yrow + 5 * QB, cell_row_ptr(fcur, A.ghost, c + 1, j + JO) + qa, bytes, bar);
+            if (have_cell) {
+                const double *yl = A.frec1 + ((size_t)j * GI + c) * FRS;
+                tma_load_1d(S + L::ylrec, yl, fbytes, bar);
+                tma_load_1d(S + L::yurec, yl + (size_t)GI * FRS, fbytes, bar);
+                tma_load_1d(S + L::crec, A.crec + ((size_t)j * GI + c) * CRS, cbytes, bar);
+            }
+            return;
+        }
         mbar_expect_tx(bar, fbytes + (have_cell ? NY * bytes + 2 * fbytes + cbytes : 0));
         tma_load_1d(S + L::xrec, A.frec0 + ((size_t)j * (GI + 1) + st) * FRS, fbytes, bar);
         if (have_cell) {
@@ -112,6 +137,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
 #define QOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * QSTEP : qo[p])
 #define MOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * MSTEP : mo[p])
     double vn[NPT], fm[NPT], fc[NPT], Fprev[NPT];
+    double hsp[TG ? NPT : 1];                                        // TG: x-face limiter result of the previous step (x-slope of the own cell for u < 0)
     bool valid[NPT];
 #pragma unroll
     for (int p = 0; p < NPT; ++p) {
@@ -119,6 +145,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         valid[p] = active && mm < mc;
         vn[p] = c_v[m0 + (mm < mc ? mm : 0)];
         Fprev[p] = 0.0;
+        if (TG) hsp[TG ? p : 0] = 0.0;
     }
     const unsigned char *ring_b = reinterpret_cast<const unsigned char *>(ring) + qb0;
     const unsigned char *stages_b = reinterpret_cast<const unsigned char *>(stages);
@@ -167,6 +194,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         const double p3 = Ek * xr[FR_C03];
         const double c4 = uk * xr[FR_MT4];
         const double c45 = uk * fma(uk, xr[FR_MT5], sgx * xr[FR_MT4]);
+        const double cx6 = TG ? uk * xr[FR_MT5T] : 0.0;              // O8t: -ell Mt5 n t theta0 on the x-face, per unit of t (h_y theta0)
         const unsigned char *xm = S + (L::xrec + FR_NCOEF + NUP) * 8 + mb0;
         const unsigned char *rn = ring_b + xslot_new * QBB;
         if (++xslot_new == NSX) xslot_new = 0;
@@ -198,7 +226,17 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
             KF = cr[CR_KF]; KD = cr[CR_KD];
             l4 = ylr[FR_MT4]; l5 = ylr[FR_MT5]; u4 = yur[FR_MT4]; u5 = yur[FR_MT5];
         }
+        // O8t on the y-faces of the own cell: t = u_k, so the coefficient of (h_x theta0) is per thread and face
+        const double cl6 = (TG && have_cell) ? uk * ylr[FR_MT5T] : 0.0, cu6 = (TG && have_cell) ? uk * yur[FR_MT5T] : 0.0;
         const unsigned char *y0 = S + L::yrow * 8 + qb0, *y1 = y0 + QBB, *y2 = y1 + QBB, *y3 = y2 + QBB;
+        // TG rows: y3 = (c-1, jn), y4 = (c+1, jn), y5 = (c+1, jo); the y-neighbours (j-1, j+1) of the x-face's upwind cell are
+        // (y1, y2) / (y0, y1) of the own column for u > 0 and (y4, y5) / (y5, y4) of column c+1 for u < 0 (v > 0 / v < 0 chunks)
+        const unsigned char *y4 = y3 + QBB, *y5 = y4 + QBB;
+        const unsigned char *tlo = posx ? (SGN > 0 ? y1 : y0) : (SGN > 0 ? y4 : y5), *thi = posx ? (SGN > 0 ? y2 : y1) : (SGN > 0 ? y5 : y4);
+        const int cown = a - 1;
+        const bool cm_miss = TG && cown == 0 && BCX0 == BC_WALL, cp_miss = TG && cown == GI - 1 && BCX1 == BC_WALL;
+        const bool nb_ghost = TG && (SGN > 0 ? (j - 1 < 0 && BCY0 == BC_FIXED) : (j + 1 >= GJ && BCY1 == BC_FIXED));
+        const bool tgb = TG && (a < 2 || a + 2 > GI || j < 1 || j > GJ - 2);      // near a boundary: take the flagged body
         const unsigned char *ylm = S + (L::ylrec + FR_NCOEF + NUP) * 8 + mb0, *yum = S + (L::yurec + FR_NCOEF + NUP) * 8 + mb0;
         const unsigned char *cgn = S + (L::crec + CR_NCOEF + 2 * NUP) * 8 + mb0, *cgp = cgn + NVP * 8;
         unsigned char *out = out_row + (size_t)max(a - 1, 0) * (NPAD * 8);
@@ -217,7 +255,17 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
                 double hs = vl_half(dmx, dpx);
                 if (FL && xmc) { fup = rwx * ldsd(gwx, QOFF(p)); hs = 0.0; }
                 const double X = fma(t, fma(t, fma(t, p3, p2), p1), p0) * ldsd(xm, MOFF(p));
-                const double F = fma(c4, fup, fma(c45, hs, X));
+                double F = fma(c4, fup, fma(c45, hs, X));
+                double hown = 0.0;                                   // TG: h_x sigma_x of the own cell a-1
+                if constexpr (TG) {
+                    // tangential slope on the x-face: limited y-slope of its upwind cell (value fc, y-neighbours tlo / thi)
+                    double dlo = fc[p] - ldsd(tlo, QOFF(p)), dhi = ldsd(thi, QOFF(p)) - fc[p];
+                    if (FL) { if (wl1) dlo = dhi; if (wu1) dhi = dlo; }
+                    const double hty = vl_half(dlo, dhi);
+                    F = fma(cx6 * t, hty, F);
+                    hown = posx ? hs : hsp[p];
+                    hsp[p] = hs;
+                }
                 const double Dx = Fprev[p] - F;
                 Fprev[p] = F;
                 const double own = posx ? fc[p] : fm[p];             // row of cell a-1
@@ -248,15 +296,25 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
                 const double b1 = useR ? qu1n : qu1, b2 = useR ? qu2n : qu2, b3 = useR ? qu3n : qu3;
                 const double Xl = fma(n, fma(n, fma(n, a3, a2), a1), ql0) * ldsd(ylm, MOFF(p));
                 const double Xu = fma(n, fma(n, fma(n, b3, b2), b1), qu0) * ldsd(yum, MOFF(p));
-                const double Gl = fma(l4, ful, fma(fma(l5, n, sg * l4), hl, Xl));
-                const double Gu = fma(u4, fuu, fma(fma(u5, n, sg * u4), hu, Xu));
+                double Gl = fma(l4, ful, fma(fma(l5, n, sg * l4), hl, Xl));
+                double Gu = fma(u4, fuu, fma(fma(u5, n, sg * u4), hu, Xu));
+                if constexpr (TG) {
+                    // tangential slopes on the y-faces: x-slope of the upwind neighbour cell (c, jn) from its staged x-neighbours,
+                    // and the own cell's x-slope
+                    double dlo = r1 - ldsd(y3, QOFF(p)), dhi = ldsd(y4, QOFF(p)) - r1;
+                    if (FL) { if (cm_miss) dlo = dhi; if (cp_miss) dhi = dlo; }
+                    double hnb = vl_half(dlo, dhi);
+                    if (FL && nb_ghost) hnb = 0.0;                   // a ghost cell has no slope (O1)
+                    Gl = fma(cl6, SGN > 0 ? hnb : hown, Gl);
+                    Gu = fma(cu6, SGN > 0 ? hown : hnb, Gu);
+                }
                 const double Dq = fma(n, Gl - Gu, Dx);
                 const double g = fma(ldsd(cgp, MOFF(p)), gpu, ldsd(cgn, MOFF(p)) * gnu);
                 const double fnw = fma(KF, own, fma(KD, Dq, g));     // P:L41 Eq. (3), solved for f^{n+1}
                 if (valid[p]) *reinterpret_cast<double *>(out + p * QSTEP) = fnw;
             }
         };
-        if (anyx || (anyy && have_cell)) body(true_c{}); else body(false_c{});
+        if (anyx || (anyy && have_cell) || tgb) body(true_c{}); else body(false_c{});
         __syncthreads();                                             // row a and stage a are consumed
         if (tid == issuer) {                                         // one lane of warp (a - c0) mod W issues the copies of two steps ahead
             if (a + 3 <= rows_last) issue_x(a + 3);
@@ -267,7 +325,10 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     }
 }
 
-static_assert(StageL<3>::BYTES == G_SMEM_UPD3 && StageL<4>::BYTES == G_SMEM_UPD4, "host mirror of the shared-memory layout (ugks_jit.cu) disagrees");
+static_assert(StageL<TG ? 6 : 3>::BYTES == G_SMEM_UPD3 && StageL<4>::BYTES == G_SMEM_UPD4, "host mirror of the shared-memory layout (ugks_jit.cu) disagrees");
+#if G_NMIX > 0
+static_assert(!TG, "the tangential reconstruction needs sorted velocity nodes (no mixed-sign chunks)");
+#endif
 
 // one launch covers the chunk range [chunk0, chunk0 + nch): the CTA dispatches on the sign class of its chunk (the two uniform
 // classes of a cell read its records while they are in the L2)

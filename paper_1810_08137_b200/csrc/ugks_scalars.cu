@@ -88,8 +88,8 @@ __device__ void cell_W_and_tgrad(const UgksParams &P, const double *W, int pos, 
 __device__ __forceinline__ void swap12(double w[4]) { const double t = w[1]; w[1] = w[2]; w[2] = t; }
 
 // raw half-range sums (set `set`) of the cell at `pos` on `line`, added over the chunks that feed that set
-template <int DIR>
-__device__ __forceinline__ void add_cell_raw(const UgksParams &P, int pos, int line, int set, double raw[NRAW])
+template <int DIR, bool TGS>
+__device__ __forceinline__ void add_cell_raw(const UgksParams &P, int pos, int line, int set, double *raw)
 {
     const size_t cell = DIR == 0 ? (size_t)line * P.I + pos : (size_t)pos * P.I + line;
     const double *cm = P.cmom + cell * P.nchunk * CMS + set * NRAW;
@@ -98,32 +98,40 @@ __device__ __forceinline__ void add_cell_raw(const UgksParams &P, int pos, int l
         const int sg = ch.z;
         if (set == 2 && sg < 0) continue;                            // a chunk of v < 0 rows holds no y+ part
         if (set == 3 && sg > 0 && !ch.w) continue;                   // ... of v > 0 rows no y- part, unless it holds the v = 0 row
-        for (int v = 0; v < NRAW; ++v) raw[v] += cm[c * CMS + v];
+        for (int v = 0; v < (TGS ? NRAW : NRAW_BASE); ++v) raw[v] += cm[c * CMS + v];
     }
 }
 
-template <int DIR>
+template <int DIR, bool TGS>
 __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
 {
+    constexpr int NR = TGS ? NRAW : NRAW_BASE;                       // raw sums in use (TGS: option "tangential")
     const size_t face = DIR == 0 ? (size_t)line * (P.I + 1) + pos : (size_t)pos * P.I + line;
     const int n = DIR == 0 ? P.I : P.J, lo = DIR == 0 ? 0 : 2;
     // O3 face sums = plus-side part of the left cell + minus-side part of the right cell (ghost rows: constants of O0)
-    double raw[NRAW];
-    for (int v = 0; v < NRAW; ++v) raw[v] = 0.0;
+    double raw[NR];
+    for (int v = 0; v < NR; ++v) raw[v] = 0.0;
     {
         int pl = pos - 1, pr = pos;
         if (pl < 0 && P.bc[lo] == BC_PERIODIC) pl += n;
         if (pr >= n && P.bc[lo + 1] == BC_PERIODIC) pr -= n;
-        if (pl >= 0) add_cell_raw<DIR>(P, pl, line, DIR == 0 ? 0 : 2, raw);
-        else if (P.bc[lo] == BC_FIXED) for (int v = 0; v < NRAW; ++v) raw[v] += P.ghostmom[lo * NRAW + v];
-        if (pr < n) add_cell_raw<DIR>(P, pr, line, DIR == 0 ? 1 : 3, raw);
-        else if (P.bc[lo + 1] == BC_FIXED) for (int v = 0; v < NRAW; ++v) raw[v] += P.ghostmom[(lo + 1) * NRAW + v];
+        if (pl >= 0) add_cell_raw<DIR, TGS>(P, pl, line, DIR == 0 ? 0 : 2, raw);
+        else if (P.bc[lo] == BC_FIXED) for (int v = 0; v < NR; ++v) raw[v] += P.ghostmom[lo * NRAW + v];
+        if (pr < n) add_cell_raw<DIR, TGS>(P, pr, line, DIR == 0 ? 1 : 3, raw);
+        else if (P.bc[lo + 1] == BC_FIXED) for (int v = 0; v < NR; ++v) raw[v] += P.ghostmom[(lo + 1) * NRAW + v];
     }
     const double ih = 2.0 / (DIR == 0 ? P.dx : P.dy);
     double M[11];
     M[0] = raw[RW_M00]; M[1] = raw[RW_M10]; M[2] = raw[RW_M01]; M[3] = 0.5 * (raw[RW_M20] + raw[RW_M02]);
     M[4] = raw[RW_M20]; M[5] = raw[RW_M11]; M[6] = 0.5 * (raw[RW_M30] + raw[RW_M12]);
     M[7] = ih * raw[RW_S20]; M[8] = ih * raw[RW_S30]; M[9] = ih * raw[RW_S21]; M[10] = ih * 0.5 * (raw[RW_S40] + raw[RW_S22]);
+    // O8t (option "tangential"): sum w n t psi theta0 from the raw sums of h_t theta0, h_t = half the TANGENTIAL spacing
+    const double iht = TGS ? 2.0 / (DIR == 0 ? P.dy : P.dx) : 0.0;
+    double Tm[4] = { 0.0, 0.0, 0.0, 0.0 };
+    if (TGS) {
+        Tm[0] = iht * raw[TGS ? RW_T11 : 0]; Tm[1] = iht * raw[TGS ? RW_T21 : 0]; Tm[2] = iht * raw[TGS ? RW_T12 : 0];
+        Tm[3] = iht * 0.5 * (raw[TGS ? RW_T31 : 0] + raw[TGS ? RW_T13 : 0]);
+    }
     double *cf = P.frec[DIR] + face * P.frs, *fw = P.fw[DIR] + face * 4;
     const double h = 0.5 * (DIR == 0 ? P.dx : P.dy), ell = DIR == 0 ? P.dy : P.dx, dt = P.dt;
 
@@ -210,6 +218,7 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
     F[1] += Mt4 * M[4] - Mt5 * M[8];
     F[2] += Mt4 * M[5] - Mt5 * M[9];
     F[3] += Mt4 * M[6] - Mt5 * M[10];
+    if (TGS) for (int r = 0; r < 4; ++r) F[r] -= Mt5 * Tm[r];
     for (int r = 0; r < 4; ++r) F[r] *= ell;
     if (DIR == 1) swap12(F);
     for (int r = 0; r < 4; ++r) fw[r] = F[r];
@@ -232,15 +241,16 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
         o[LR_C11] = sc * (Mt2 * (a[2] + bb[1]));
         o[LR_C12] = sc * (0.5 * Mt2 * a[3]);
     }
-    cf[23] = 0.0;
+    cf[FR_MT5T] = -ell * Mt5 * iht;
 }
 
+template <bool TGS>
 __global__ void __launch_bounds__(128) k_face_scalars(const UgksParams P, const int cur)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     const int nfx = nfaces_x(P), nfy = nfaces_y(P);
-    if (t < nfx) face_scalars<0>(P, cur, t % (P.I + 1), t / (P.I + 1));
-    else if (t < nfx + nfy) { const int s = t - nfx; face_scalars<1>(P, cur, s / P.I, s % P.I); }
+    if (t < nfx) face_scalars<0, TGS>(P, cur, t % (P.I + 1), t / (P.I + 1));
+    else if (t < nfx + nfy) { const int s = t - nfx; face_scalars<1, TGS>(P, cur, s / P.I, s % P.I); }
 }
 
 // U1 + U2 per cell, plus the partial sums of the residual (O11)
@@ -398,7 +408,8 @@ int launch_poison_smem(cudaStream_t st)
 int launch_face_scalars(const UgksParams &P, int cur, cudaStream_t st)
 {
     const int n = nfaces_x(P) + nfaces_y(P);
-    k_face_scalars<<<(n + 127) / 128, 128, 0, st>>>(P, cur);
+    if (P.tangential) k_face_scalars<true><<<(n + 127) / 128, 128, 0, st>>>(P, cur);
+    else k_face_scalars<false><<<(n + 127) / 128, 128, 0, st>>>(P, cur);
     return 1;
 }
 int launch_cell_scalars(const UgksParams &P, int cur, int resblocks, cudaStream_t st)

@@ -25,7 +25,7 @@ def _run_pair(p, steps, W=None, f=None, threads=8, options=()):
     from paper_1810_08137_b200 import Ugks
     if W is None:
         W, f, _ = workloads.initial_state(p)
-    o = Oracle(p, threads=threads)
+    o = Oracle(p, threads=threads, tangential=any(k == "tangential" and v for k, v in options))
     o.set_state(W, f)
     g = Ugks(p)
     for name, value in options:
@@ -79,6 +79,75 @@ def test_stale_shared_memory_is_never_read(name, I, J, nuv):
     ragged chunks of 49x49 / 69x69 grids, the one-row v = 0 chunk) or a ragged strip that read shared memory the CTA has not
     written would poison the sums.  Three steps, so that both parities of every double buffer are used."""
     _check(_run_pair(workloads.channel_config(name, I=I, J=J, Nuv=nuv), 3, options=(("poison", 1),)), 3 * TOL_1)
+
+
+TG = (("tangential", 1),)
+
+
+@pytest.mark.parametrize("steps,tol", [(1, TOL_1), (10, TOL_100)])
+def test_tangential_C1_channel(steps, tol):
+    """NEXT-1 (O3t/O8t): the tangential slope of f in the free-transport part, GPU vs oracle on the C1 channel (fixed in x, walls in y)."""
+    _check(_run_pair(workloads.channel_config("C1"), steps, options=TG), tol)
+
+
+@pytest.mark.parametrize("name,I,J,nuv", [("C3", 40, 12, None), ("C4", 37, 9, None), ("C5", 6, 5, None), ("C2", 33, 4, 29), ("C2", 36, 5, 69),
+                                          ("C1", 2, 2, 6), ("C1", 3, 2, 6), ("C1", 33, 2, 12)])
+def test_tangential_velocity_grids_ragged_meshes_poisoned(name, I, J, nuv):
+    """every config's velocity grid, odd grids with a v = 0 row, ragged strips and minimal meshes with the tangential slopes on;
+    shared memory poisoned (the three extra staged rows of k_flux_update must cover every read)."""
+    _check(_run_pair(workloads.channel_config(name, I=I, J=J, Nuv=nuv), 3, options=TG + (("poison", 1),)), 3 * TOL_1)
+
+
+def test_tangential_periodic_walls_and_fixed_sides():
+    """periodic box (odd grid), closed box with moving walls, and fixed sides in y with walls in x (the ghost cells of a FIXED
+    side have no slope; next to a wall the tangential neighbour slope is one-sided)."""
+    p = workloads.periodic_box(9, 7, 13, 9, a=5.0, Kn=0.05, seed=5, bu=6.0, lx=1.3, ly=0.7)
+    _check(_run_pair(p, 3, options=TG), 3 * TOL_1)
+    u, wu = workloads.trapezoid_grid(17, 6.0)
+    wall = (workloads.BC_WALL, 1.0, 0.1, -0.05, 1.2)
+    p = workloads.Problem(I=6, J=5, x0=0.0, x1=1.0, y0=0.0, y1=1.0, u=u, wu=wu, v=u.copy(), wv=wu.copy(), Kn=0.1,
+                          bcs=[wall] * 4, cfl=0.8, seed=9, eps=(0.05, 0.05, 0.05, 0.05), rho_drop=0.0)
+    _check(_run_pair(p, 4, options=TG), 4 * TOL_1)
+    p = workloads.channel_config("C1", I=7, J=11, Nuv=14)
+    p.bcs = [p.bcs[2], p.bcs[3], (workloads.BC_FIXED, 1.0, 0.0, 0.05, 1.0), (workloads.BC_FIXED, 0.9, 0.0, 0.0, 1.1)]
+    _check(_run_pair(p, 3, options=TG), 3 * TOL_1)
+    # rough data: both limiters active everywhere, stiff / collisionless
+    rng = np.random.default_rng(3)
+    for kn in (1e-5, 1e9):
+        p = workloads.periodic_box(8, 6, 16, 16, a=6.0, Kn=kn, seed=4)
+        W, f, _ = workloads.initial_state(p)
+        f = f * rng.uniform(0.5, 1.5, f.shape)
+        _check(_run_pair(p, 2, W, f, options=TG), 2 * TOL_1)
+    # fixed sides in BOTH directions (corner ghosts: the x side takes precedence, O1)
+    p = workloads.channel_config("C1", I=6, J=5, Nuv=10)
+    p.bcs = [p.bcs[0], p.bcs[1], (workloads.BC_FIXED, 1.0, 0.0, 0.05, 1.0), (workloads.BC_FIXED, 0.9, 0.0, 0.0, 1.1)]
+    _check(_run_pair(p, 3, options=TG), 3 * TOL_1)
+
+
+def test_tangential_needs_sign_uniform_chunks_and_can_be_switched_off():
+    from paper_1810_08137_b200 import Ugks, UgksError
+    p = workloads.periodic_box(7, 5, 12, 10, a=5.0, Kn=0.1, seed=12)
+    pv = np.array([0, 9, 1, 8, 2, 7, 3, 6, 4, 5])             # signs alternate: more runs than sign-uniform chunks are made for
+    p.v, p.wv = p.v[pv], p.wv[pv]
+    g = Ugks(p)
+    with pytest.raises(UgksError):
+        g.set_option("tangential", 1)                         # mixed-sign chunks: refused
+    p2 = workloads.periodic_box(7, 5, 12, 10, a=5.0, Kn=0.1, seed=12)
+    pv = np.array([5, 6, 7, 8, 9, 4, 3, 2, 1, 0])             # not ascending, but two sign-uniform runs: fine
+    p2.v, p2.wv = p2.v[pv], p2.wv[pv]
+    pu = np.random.default_rng(1).permutation(12)
+    p2.u, p2.wu = p2.u[pu], p2.wu[pu]
+    _check(_run_pair(p2, 3, options=TG), 3 * TOL_1)
+    q = workloads.channel_config("C1")
+    W, f, _ = workloads.initial_state(q)
+    outs = []
+    for toggle in (False, True):
+        h = Ugks(q)
+        if toggle:
+            h.set_option("tangential", 1); h.set_option("tangential", 0)
+        h.set_state(W, f); h.step(3)
+        outs.append(h.f())
+    assert np.array_equal(outs[0], outs[1])
 
 
 @pytest.mark.parametrize("nu,nv", [(29, 29), (13, 9), (7, 33), (16, 12)])
@@ -182,6 +251,28 @@ def _host_ram_or_skip(p, copies, what):
 # C4 50).  On the 16-core GPU box the oracle needs ~7 s per C4 step, so C4 alone takes ~6 of the suite's ~10 minutes;
 # UGKS_PARITY_C4_STEPS=<n> shortens it.
 _FULL = [("C2", (1, 200)), ("C3", (1, 100)), ("C5", (1, 50)), ("C4", (1, 50))]
+
+
+@pytest.mark.parametrize("name,checkpoints", [("C2", (1, 50)), ("C3", (1, 20))])
+def test_full_size_full_field_tangential(name, checkpoints):
+    """NEXT-1 at BASELINE.json's sizes: the whole field with the tangential slopes on (default launch geometry of that mode)."""
+    import os
+    from oracle import Oracle
+    from paper_1810_08137_b200 import Ugks
+    p = workloads.channel_config(name)
+    _host_ram_or_skip(p, 5.5, "the oracle state (2 copies), the input and the two outputs")
+    W, f, _ = workloads.initial_state(p)
+    g = Ugks(p, tangential=True)
+    g.set_state(W, f)
+    o = Oracle(p, threads=os.cpu_count() or 8, tangential=True)
+    o.set_state(W, f)
+    del f
+    done = 0
+    for n in checkpoints:
+        g.step(n - done)
+        o.step(n - done)
+        done = n
+        _check(_compare(g, o), TOL_1 if n == 1 else TOL_100)
 
 
 @pytest.mark.parametrize("name,checkpoints", _FULL)

@@ -57,7 +57,7 @@ struct UgksParams {
     const int4 *chunks;              // [nchunk] (m0, mc, sign of v over the chunk: +1 / -1 / 0 = mixed, 1 if row m0 is a v = 0 row of a +1 chunk)
     double *f[2];                    // ping-pong copies of f, rows padded to Npad
     double *W[2];                    // ping-pong copies of W [cells][4]
-    double *cmom;                    // [cells][nchunk][NSET][NRAW]
+    double *cmom;                    // [cells][nchunk][CMS]: 4 sets x 13 base sums, then 4 sets x 5 T sums
     double *frec[2];                 // [faces][frs], x then y faces
     double *fw[2];                   // [faces][4] time-integrated macroscopic flux, global frame
     double *crec;                    // [cells][crs]

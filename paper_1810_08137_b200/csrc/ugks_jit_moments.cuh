@@ -188,10 +188,10 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
         const int idx = v % NRK;
         o_first[q] = set < 2 ? v * L::NSX : 2 * NRK * L::NSX + (v - 2 * NRK) * L::NSY;
         if (!MIXED && set >= 2) set = ch.z > 0 ? 2 : 3;
-        o_dst[q] = set * NRAW + idx;
+        o_dst[q] = idx < 13 ? set * 13 + idx : 52 + set * 5 + (idx - 13);    // [4 sets x 13 base sums | 4 sets x 5 T sums]
         if (!MIXED && v >= 3 * NRK) {                                // the three y- outputs of the v = 0 row (flagged chunk only)
             const int e = v - 3 * NRK;
-            o_dst[q] = ch.w ? 3 * NRAW + (e == 0 ? RW_M00 : (e == 1 ? RW_M01 : RW_M02)) : -1;
+            o_dst[q] = ch.w ? 3 * 13 + (e == 0 ? RW_M00 : (e == 1 ? RW_M01 : RW_M02)) : -1;
         }
     }
     __syncthreads();

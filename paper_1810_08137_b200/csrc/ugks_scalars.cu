@@ -92,13 +92,16 @@ template <int DIR, bool TGS>
 __device__ __forceinline__ void add_cell_raw(const UgksParams &P, int pos, int line, int set, double *raw)
 {
     const size_t cell = DIR == 0 ? (size_t)line * P.I + pos : (size_t)pos * P.I + line;
-    const double *cm = P.cmom + cell * P.nchunk * CMS + set * NRAW;
+    // per (cell, chunk): [4 sets x 13 base sums | 4 sets x 5 T sums (option "tangential")]
+    const double *cm = P.cmom + cell * P.nchunk * CMS + set * NRAW_BASE;
+    const double *ct = P.cmom + cell * P.nchunk * CMS + NSET * NRAW_BASE + set * (NRAW - NRAW_BASE);
     for (int c = 0; c < P.nchunk; ++c) {
         const int4 ch = P.chunks[c];
         const int sg = ch.z;
         if (set == 2 && sg < 0) continue;                            // a chunk of v < 0 rows holds no y+ part
         if (set == 3 && sg > 0 && !ch.w) continue;                   // ... of v > 0 rows no y- part, unless it holds the v = 0 row
-        for (int v = 0; v < (TGS ? NRAW : NRAW_BASE); ++v) raw[v] += cm[c * CMS + v];
+        for (int v = 0; v < NRAW_BASE; ++v) raw[v] += cm[c * CMS + v];
+        if (TGS) for (int v = NRAW_BASE; v < NRAW; ++v) raw[TGS ? v : 0] += ct[c * CMS + v - NRAW_BASE];
     }
 }
 

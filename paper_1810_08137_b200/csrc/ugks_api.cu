@@ -361,6 +361,16 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     }
     if (!(P.mu_ref > 0.0)) { free(c); return fail(nullptr, UGKS_EINVAL, "%s", "mu_ref / Kn must be positive"); }
     for (int s = 0; s < 4; ++s) P.bc[s] = b[s]->type;
+    {   // equally spaced nodes (to 4 ulp of the largest node)?  then k_tables runs its exponentials as a two-term recurrence
+        auto spacing = [](const double *x, int n) {
+            if (n < 3) return 0.0;
+            const double h = (x[n - 1] - x[0]) / (n - 1);
+            double mx = 0.0, dev = 0.0;
+            for (int k = 0; k < n; ++k) { mx = fmax(mx, fabs(x[k])); dev = fmax(dev, fabs(x[k] - (x[0] + k * h))); }
+            return (h > 0.0 && dev <= 4.0 * 2.220446049250313e-16 * mx) ? h : 0.0;
+        };
+        P.hu = spacing(vg->u, vg->Nu); P.hv = spacing(vg->v, vg->Nv);
+    }
     char *base = (char *)workspace_dev;
     auto D = [&](size_t off) { return (double *)(base + off); };
     P.f[0] = D(L.f[0]); P.f[1] = D(L.f[1]); P.W[0] = D(L.W[0]); P.W[1] = D(L.W[1]);

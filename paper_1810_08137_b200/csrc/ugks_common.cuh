@@ -46,6 +46,7 @@ struct UgksParams {
     int NuP, NvP;                    // Nu, Nv rounded up to even (16-byte aligned table segments)
     int frs, crs;                    // record strides in doubles: FR_NCOEF + NuP + NvP, CR_NCOEF + 2 NuP + 2 NvP
     double dx, dy, dt, omega, mu_ref;
+    double hu, hv;                   // spacing of the u / v nodes if they are equally spaced (to a few ulp), else 0 (k_tables)
     int bc[4];                       // xmin, xmax, ymin, ymax
     int tangential;                  // option "tangential" (NEXT-1, O3t/O8t): f is reconstructed in the tangential direction too
     const double *u, *wu, *v, *wv;   // device copies of the velocity nodes / weights

@@ -435,52 +435,77 @@ int launch_setup(const UgksParams &P, const double *bc_prims, double *ghost, dou
 // ---------------------------------------------------------------------------------------------
 // k_tables: every exponential of the step (S6 and the two cell equilibria of U2), once per face / cell and node:
 // exp(-lam ((u-U)^2 + (v-V)^2)) = E_k[k] E_m[m] on the tensor-product grid, so a face needs Nu + Nv exponentials, not Nu Nv.
-// One thread per table entry; a block owns TPB consecutive tables (a face Maxwellian, g^n of a cell, g^{n+1} of a cell), so
-// the entry -> (table, node) split is 32-bit arithmetic on small numbers and the stores of a warp are contiguous.  The
-// records are read back by k_flux_update through TMA.
-constexpr int TPB = 16;                                              // tables per block
+// One thread per SEGMENT of 8 consecutive entries of one table (a face Maxwellian, g^n of a cell, g^{n+1} of a cell) and
+// direction.  Where the nodes of that direction are equally spaced (P.hu / P.hv > 0, checked at init) the segment costs three
+// exponentials instead of eight: with x_i = x_s + i h,  E_{i+1} = E_i D_i,  D_{i+1} = D_i Q,  E_s = exp(-lam (x_s - c)^2),
+// D_s = exp(-lam h (2 (x_s - c) + h)),  Q = exp(-2 lam h^2); seven steps add at most ~30 roundings (3e-15 relative).  Segments in
+// the far tail (E_s or D_s outside the normal range) and unequally spaced nodes take the direct exponentials.
+constexpr int TSEG = 8;
 __global__ void __launch_bounds__(256) k_tables(const UgksParams P)
 {
-    const unsigned nt = P.NuP + P.NvP;                               // entries per Maxwellian
+    const unsigned nsu = (P.NuP + TSEG - 1) / TSEG, nsv = (P.NvP + TSEG - 1) / TSEG, nseg = nsu + nsv;
     const long nfx = nfaces_x(P), nfy = nfaces_y(P), ncell = (long)P.I * P.J;
-    const long total = nfx + nfy + 2 * ncell;
-    for (long rec0 = (long)blockIdx.x * TPB; rec0 < total; rec0 += (long)gridDim.x * TPB) {
-        for (unsigned i = threadIdx.x; i < TPB * nt; i += blockDim.x) {
-            const unsigned rl = i / nt, e = i - rl * nt;
+    const long ntab = nfx + nfy + 2 * ncell;
+    constexpr unsigned TPB = 16;                                     // tables per block pass
+    for (long rec0 = (long)blockIdx.x * TPB; rec0 < ntab; rec0 += (long)gridDim.x * TPB) {
+        for (unsigned i = threadIdx.x; i < TPB * nseg; i += blockDim.x) {
+            const unsigned rl = i / nseg, sg = i - rl * nseg;
             const long rec = rec0 + rl;
-            if (rec >= total) break;
-            const bool isk = e < (unsigned)P.NuP;
-            const int idx = isk ? e : e - P.NuP;
-            const bool pad = isk ? idx >= P.Nu : idx >= P.Nv;
-            const double node = pad ? 0.0 : (isk ? P.u[idx] : P.v[idx]);
+            if (rec >= ntab) break;
+            const bool isk = sg < nsu;
+            const int e0 = (isk ? sg : sg - nsu) * TSEG, nn = isk ? P.Nu : P.Nv, np = isk ? P.NuP : P.NvP;
+            const double *node = isk ? P.u : P.v;
+            const double h = isk ? P.hu : P.hv;
             double lam, cen, pref = 1.0, *dst;
-            bool zero = pad;
+            bool zero = false;
             if (rec < nfx + nfy) {                                   // face Maxwellian (local frame: U normal, V tangential)
                 const int dir = rec >= nfx;
                 double *fr = P.frec[dir] + (dir ? rec - nfx : rec) * P.frs;
                 lam = fr[FR_LAM];
                 cen = (isk == (dir == 0)) ? fr[FR_U] : fr[FR_V];     // x-face: u is normal; y-face: v is normal
-                zero = zero || fr[FR_TYPE] != 0.0;                   // wall faces carry no equilibrium part
-                dst = fr + FR_NCOEF + e;
+                zero = fr[FR_TYPE] != 0.0;                           // wall faces carry no equilibrium part
+                dst = fr + FR_NCOEF + (isk ? 0 : P.NuP) + e0;
             } else {                                                 // cell equilibria g^n (w = 0), g^{n+1} (w = 1)
                 const long cw = rec - nfx - nfy, cell = cw >> 1;
                 const int w = (int)(cw & 1);
                 double *cr = P.crec + cell * P.crs;
                 lam = cr[w ? CR_LP : CR_LN];
                 cen = isk ? cr[w ? CR_UP : CR_UN] : cr[w ? CR_VP : CR_VN];
-                if (isk) pref = cr[w ? CR_GP : CR_GN];
-                dst = cr + CR_NCOEF + (isk ? w * P.NuP + idx : 2 * P.NuP + w * P.NvP + idx);
+                if (isk) pref = cr[w ? CR_GP : CR_GN];               // relaxation prefactor folded into the u-table
+                dst = cr + CR_NCOEF + (isk ? w * P.NuP : 2 * P.NuP + w * P.NvP) + e0;
             }
-            const double d = node - cen;
-            *dst = zero ? 0.0 : pref * exp(-lam * d * d);
+            const int cnt = min(TSEG, np - e0);                      // entries of this segment (np is even: cnt is even)
+            double val[TSEG];
+            bool done = false;
+            if (!zero && h > 0.0 && e0 < nn) {
+                const double x = node[e0] - cen;
+                const double E = exp(-lam * x * x), D = exp(-lam * h * (2.0 * x + h)), Q = exp(-2.0 * lam * h * h);
+                if (E > 1e-200 && D > 1e-100 && D < 1e100) {         // everything stays a normal number over the segment
+                    double Ei = pref * E, Di = D;
+#pragma unroll
+                    for (int q = 0; q < TSEG; ++q) { val[q] = e0 + q < nn ? Ei : 0.0; Ei *= Di; Di *= Q; }
+                    done = true;
+                }
+            }
+            if (!done) {
+#pragma unroll
+                for (int q = 0; q < TSEG; ++q) {
+                    const int idx = e0 + q;
+                    const double d = (idx < nn ? node[idx] : 0.0) - cen;
+                    val[q] = (zero || idx >= nn) ? 0.0 : pref * exp(-lam * d * d);
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < TSEG; q += 2)
+                if (q < cnt) *reinterpret_cast<double2 *>(dst + q) = make_double2(val[q], val[q + 1]);
         }
     }
 }
 
 int launch_tables(const UgksParams &P, cudaStream_t st)
 {
-    const long total = (long)nfaces_x(P) + nfaces_y(P) + 2L * P.I * P.J;
-    long blocks = (total + TPB - 1) / TPB;
+    const long ntab = (long)nfaces_x(P) + nfaces_y(P) + 2L * P.I * P.J;
+    long blocks = (ntab + 15) / 16;
     if (blocks > 148L * 128) blocks = 148L * 128;
     k_tables<<<(int)blocks, 256, 0, st>>>(P);
     return 1;

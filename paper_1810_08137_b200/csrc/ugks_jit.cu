@@ -30,9 +30,21 @@ int cdivi(int a, int b) { return (a + b - 1) / b; }
 
 // host mirrors of MomL<MIXED>::BYTES and StageL<NY>::BYTES (the device code static_asserts that they agree)
 int nsxm() { const char *e = getenv("UGKS_NSXM"); const int n = e ? atoi(e) : 3; return n < 2 ? 2 : (n > 4 ? 4 : n); }   // x-ring slots of k_cell_moments
-int smem_mom(const UgksParams &P, const KGeom &G, bool mixed)
+int smem_mom_q(const UgksParams &P, const KGeom &G, bool mixed, int QB);
+int smem_upd_q(const UgksParams &P, const KGeom &G, int ny, int QB);
+int upd_rows(const UgksParams &P, const KGeom &G) { return G.nmix > 0 ? 4 : (P.tangential ? 6 : 3); }
+// slot size of a staged chunk: MC*NU + 1 doubles rounded up to even, or to a 128-byte multiple if no resident CTA is lost to it
+int qb_of(int kind, const UgksParams &P, const KGeom &G)
 {
-    const int BT = (P.Nu * G.R + 31) / 32 * 32, QB = pad2i(G.cmax * P.Nu + 1);
+    const int q2 = pad2i(G.cmax * P.Nu + 1), q16 = (G.cmax * P.Nu + 1 + 15) & ~15;
+    const int s2 = kind == JIT_MOMENTS ? smem_mom_q(P, G, G.nmix > 0, q2) : smem_upd_q(P, G, upd_rows(P, G), q2);
+    const int s16 = kind == JIT_MOMENTS ? smem_mom_q(P, G, G.nmix > 0, q16) : smem_upd_q(P, G, upd_rows(P, G), q16);
+    return (227 * 1024) / (s16 + 1024) == (227 * 1024) / (s2 + 1024) ? q16 : q2;
+}
+int smem_mom(const UgksParams &P, const KGeom &G, bool mixed) { return smem_mom_q(P, G, mixed, qb_of(JIT_MOMENTS, P, G)); }
+int smem_mom_q(const UgksParams &P, const KGeom &G, bool mixed, int QB)
+{
+    const int BT = (P.Nu * G.R + 31) / 32 * 32;
     bool zrow = false;
     for (const int4 &c : G.chunks) if (c.w) zrow = true;
     const int nrk = P.tangential ? 18 : 13;
@@ -45,9 +57,9 @@ int smem_mom(const UgksParams &P, const KGeom &G, bool mixed)
                       pad2i(2 * nitem) + nsxm() + 3;
     return total * 8;
 }
-int smem_upd(const UgksParams &P, const KGeom &G, int ny)
+int smem_upd(const UgksParams &P, const KGeom &G, int ny) { return smem_upd_q(P, G, ny, qb_of(JIT_UPDATE, P, G)); }
+int smem_upd_q(const UgksParams &P, const KGeom &G, int ny, int QB)
 {
-    const int QB = pad2i(G.cmax * P.Nu + 1);
     const int size = ny * QB + 3 * P.frs + P.crs;
     return (3 * QB + 2 * size) * 8 + 5 * 8;
 }
@@ -112,7 +124,7 @@ std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const dou
     DEF("G_BC0", P.bc[0]); DEF("G_BC1", P.bc[1]); DEF("G_BC2", P.bc[2]); DEF("G_BC3", P.bc[3]);
     DEF("G_NCHUNK", G.nchunk()); DEF("G_NMIX", G.nmix); DEF("G_MC", G.cmax); DEF("G_R", G.R); DEF("G_NPT", G.npt); DEF("G_STRIP", G.strip);
     { int z = 0; for (const int4 &c : G.chunks) if (c.w) z = 1; DEF("G_HAS_ZROW", z); }
-    DEF("G_TANGENTIAL", P.tangential ? 1 : 0);
+    DEF("G_TANGENTIAL", P.tangential ? 1 : 0); DEF("G_QB", qb_of(kind, P, G));
     DEF("G_KXM_END", P.kxm_end); DEF("G_KXP_BEGIN", P.kxp_begin); DEF("G_RAGGED", G.ragged() ? 1 : 0);
     if (kind == JIT_MOMENTS) {
         const int sm_u = smem_mom(P, G, false), sm_m = smem_mom(P, G, true);

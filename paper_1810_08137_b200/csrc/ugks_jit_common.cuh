@@ -29,7 +29,10 @@ constexpr int NSTRIP = (GI + STRIP - 1) / STRIP;
 constexpr int BT = ((NU * R + 31) / 32) * 32;                         // compute threads of a CTA; one more warp produces (TMA)
 constexpr int KXM_END = G_KXM_END, KXP_BEGIN = G_KXP_BEGIN;          // columns with u_k <= 0: [0, KXM_END); u_k >= 0: [KXP_BEGIN, NU)
 constexpr int pad2c(int x) { return (x + 1) & ~1; }
-constexpr int QB = pad2c(MC * NU + 1);                                // doubles per staged chunk of a row (16-byte aligned start + shift)
+constexpr int QB = G_QB;                                              // doubles per staged chunk of a row: >= MC*NU + 1 (shift of an odd start), even;
+                                                                      // a 128-byte multiple where that costs no resident CTA (a warp's 256 contiguous
+                                                                      // bytes then span two shared-memory lines, not three)
+static_assert(QB >= MC * NU + 1 && QB % 2 == 0, "slot size");
 constexpr int QBB = QB * 8;
 
 // per-(cell, chunk) half-range raw moment sets (see ugks_common.cuh): sets 0 = x+, 1 = x-, 2 = y+, 3 = y-

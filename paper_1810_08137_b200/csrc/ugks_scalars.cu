@@ -248,7 +248,10 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
 }
 
 template <bool TGS>
-__global__ void __launch_bounds__(128) k_face_scalars(const UgksParams P, const int cur)
+#ifndef UGKS_FS_MINB
+#define UGKS_FS_MINB 3
+#endif
+__global__ void __launch_bounds__(128, UGKS_FS_MINB) k_face_scalars(const UgksParams P, const int cur)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     const int nfx = nfaces_x(P), nfy = nfaces_y(P);

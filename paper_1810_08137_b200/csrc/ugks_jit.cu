@@ -167,8 +167,9 @@ int jit_compile(int kind, const std::string &prelude, std::vector<char> *cubin, 
     cubin->resize(n);
     nvrtcGetCUBIN(prog, cubin->data());
     nvrtcDestroyProgram(&prog);
-    if (const char *dump = getenv("UGKS_JIT_DUMP")) {               // developer aid: keep the image for cuobjdump -sass
-        if (FILE *f = fopen(dump, "wb")) { fwrite(cubin->data(), 1, cubin->size(), f); fclose(f); }
+    if (const char *dump = getenv("UGKS_JIT_DUMP")) {               // keep the image for cuobjdump -sass: <dump>.moments.cubin / <dump>.update.cubin
+        const std::string path = std::string(dump) + (kind == JIT_MOMENTS ? ".moments.cubin" : ".update.cubin");
+        if (FILE *f = fopen(path.c_str(), "wb")) { fwrite(cubin->data(), 1, cubin->size(), f); fclose(f); }
     }
     return n ? 0 : 1;
 }

@@ -17,7 +17,8 @@ __device__ __forceinline__ Prim prim_of(const double W[4])
 }
 __device__ __forceinline__ double tau_of(const UgksParams &P, double rho, double lam)
 {
-    return 2.0 * P.mu_ref * pow(lam, 1.0 - P.omega) / rho;          // AMB-7
+    // AMB-7: tau = 2 mu_ref lam^(1-omega) / rho; the power as exp((1-omega) log lam) (lam > 0; a few ulp, half the cost of pow)
+    return 2.0 * P.mu_ref * exp((1.0 - P.omega) * log(lam)) / rho;
 }
 
 // <n^a t^b (c.psi)> for the normal-moment set X (full or half range) and tangential set Y
@@ -44,6 +45,22 @@ __device__ __forceinline__ void micro_slope(const Prim &p, const double s[4], do
     c[0] = s[0] / p.rho - p.U * c[1] - p.V * c[2] - 0.5 * (q2 + il) * c[3];
 }
 
+// the same with the reciprocals of rho and lambda formed once per face (four solves per face share them)
+struct PrimR { double U, V, lam, k, ir, il, q2; };
+__device__ __forceinline__ PrimR primr_of(const Prim &p)
+{
+    PrimR r;
+    r.U = p.U; r.V = p.V; r.lam = p.lam; r.ir = 1.0 / p.rho; r.il = 1.0 / p.lam; r.k = 2.0 * p.lam * r.ir; r.q2 = p.U * p.U + p.V * p.V;
+    return r;
+}
+__device__ __forceinline__ void micro_slope(const PrimR &p, const double s[4], double c[4])
+{
+    c[3] = p.k * p.lam * (2.0 * s[3] - 2.0 * p.U * s[1] - 2.0 * p.V * s[2] + s[0] * (p.q2 - p.il));
+    c[2] = p.k * (s[2] - p.V * s[0]) - p.V * c[3];
+    c[1] = p.k * (s[1] - p.U * s[0]) - p.U * c[3];
+    c[0] = s[0] * p.ir - p.U * c[1] - p.V * c[2] - 0.5 * (p.q2 + p.il) * c[3];
+}
+
 // W and tangential gradient of W (AMB-14) of the cell at `pos` on `line`, in the GLOBAL frame.
 // kind: 0 cell, 1 ghost, 2 wall(missing)
 template <int DIR>
@@ -67,7 +84,7 @@ __device__ void cell_W_and_tgrad(const UgksParams &P, const double *W, int pos, 
     // tangential direction: y for x-faces, x for y-faces
     const int nt = DIR == 0 ? P.J : P.I, tl = DIR == 0 ? 2 : 0;
     const int tp = DIR == 0 ? j : i;
-    const double D = DIR == 0 ? P.dy : P.dx;
+    const double iD = 1.0 / (DIR == 0 ? P.dy : P.dx);
     const double *wm = nullptr, *wp = nullptr;
     int km = 0, kp = 0;                                              // 0 cell/ghost present, 2 wall
     {
@@ -79,9 +96,9 @@ __device__ void cell_W_and_tgrad(const UgksParams &P, const double *W, int pos, 
         if (!wp && !kp) wp = W + (DIR == 0 ? ((size_t)t * P.I + i) : ((size_t)j * P.I + t)) * 4;
     }
     for (int r = 0; r < 4; ++r) {
-        if (!km && !kp) g[r] = (wp[r] - wm[r]) / (2.0 * D);
-        else if (km && !kp) g[r] = (wp[r] - w0[r]) / D;
-        else if (kp && !km) g[r] = (w0[r] - wm[r]) / D;
+        if (!km && !kp) g[r] = (wp[r] - wm[r]) * (0.5 * iD);
+        else if (km && !kp) g[r] = (wp[r] - w0[r]) * iD;
+        else if (kp && !km) g[r] = (w0[r] - wm[r]) * iD;
     }
 }
 
@@ -164,13 +181,16 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
     double W0[4] = { M[0], M[1], M[2], M[3] };
     const Prim p0 = prim_of(W0);
     if (!(p0.rho > 0.0) || !(p0.lam > 0.0)) atomicOr(P.status, 1);
+    const PrimR pr = primr_of(p0);
     // S2: Maxwellian moments (O4)
     double XL[7], XR[7], XF[7], Y[7];
     {
-        const double sl = sqrt(p0.lam), e = 0.5 * exp(-p0.lam * p0.U * p0.U) / sqrt(UGKS_PI * p0.lam);
-        const double il2 = 0.5 / p0.lam;
-        XL[0] = 0.5 * erfc(-sl * p0.U); XL[1] = p0.U * XL[0] + e;
-        XR[0] = 0.5 * erfc(sl * p0.U);  XR[1] = p0.U * XR[0] - e;
+        const double sl = sqrt(p0.lam), e = 0.5 * exp(-p0.lam * p0.U * p0.U) * pr.il * sl * 0.5641895835477562869;   // 1/sqrt(pi lam)
+        const double il2 = 0.5 * pr.il;
+        // the two half-range zeroth moments: the smaller one from erfc of a positive argument, the other as its complement
+        const double z = sl * p0.U, small = 0.5 * erfc(fabs(z));
+        XL[0] = z >= 0.0 ? 1.0 - small : small; XL[1] = p0.U * XL[0] + e;
+        XR[0] = z >= 0.0 ? small : 1.0 - small; XR[1] = p0.U * XR[0] - e;
         Y[0] = 1.0; Y[1] = p0.V;
         for (int q = 0; q < 5; ++q) {
             XL[q + 2] = p0.U * XL[q + 1] + (q + 1) * il2 * XL[q];
@@ -197,16 +217,16 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
     // S4: micro-slopes (O6)
     double sL[4], sR[4], sb[4], aL[4], aR[4], bb[4], A[4];
     for (int r = 0; r < 4; ++r) {
-        sL[r] = (W0[r] - WL[r]) / h;
-        sR[r] = (WR[r] - W0[r]) / h;
+        sL[r] = (W0[r] - WL[r]) * ih;                                // ih = 1 / h
+        sR[r] = (WR[r] - W0[r]) * ih;
         sb[r] = 0.5 * (gL[r] + gR[r]);
     }
-    micro_slope(p0, sL, aL); micro_slope(p0, sR, aR); micro_slope(p0, sb, bb);
+    micro_slope(pr, sL, aL); micro_slope(pr, sR, aR); micro_slope(pr, sb, bb);
     double sA[4] = { 0, 0, 0, 0 };
     add_T(sA, -p0.rho, XL, Y, aL, 1, 0);
     add_T(sA, -p0.rho, XR, Y, aR, 1, 0);
     add_T(sA, -p0.rho, XF, Y, bb, 0, 1);
-    micro_slope(p0, sA, A);
+    micro_slope(pr, sA, A);
     // S5: hydrodynamic flux (O7) + the free-transport sums of S7 (O8)
     double F[4];
     F[0] = p0.rho * Mt1 * XF[1];
@@ -229,7 +249,7 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
     // flux polynomial ell C0 [Mt1 + Mt2 (n a.psi + t b.psi) + Mt3 A.psi] = sum c_ab n^a t^b, C0 = rho lam / pi
     const double sc = ell * p0.rho * p0.lam / UGKS_PI;
     cf[FR_LAM] = p0.lam; cf[FR_U] = p0.U; cf[FR_V] = p0.V; cf[FR_TYPE] = 0.0; cf[FR_RHOW] = 0.0;
-    cf[FR_MT4] = ell * Mt4; cf[FR_MT5] = -ell * Mt5 * (1.0 / h); cf[FR_TAU] = tau;
+    cf[FR_MT4] = ell * Mt4; cf[FR_MT5] = -ell * Mt5 * ih; cf[FR_TAU] = tau;
     cf[FR_C00] = sc * (Mt1 + Mt3 * A[0]);
     cf[FR_C01] = sc * (Mt2 * bb[0] + Mt3 * A[2]);
     cf[FR_C02] = sc * (Mt2 * bb[2] + 0.5 * Mt3 * A[3]);

@@ -67,6 +67,7 @@ static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 // is uniform over a CTA), each run into equal chunks of at most `cm_target` rows; rows with v = 0 and, if the node order makes
 // too many runs, everything, go to "mixed" chunks that select the side per point.  Order: [v < 0][v > 0][mixed].
 constexpr int MAXCHUNK = 4096;
+constexpr int MAXNU = 512;                                           // one thread per column: a CTA of <= 512 threads keeps 128 registers per thread
 
 static void make_chunks(const double *v, int Nv, int Nu, int cm_target, KGeom *G)
 {
@@ -109,7 +110,7 @@ static void make_chunks(const double *v, int Nv, int Nu, int cm_target, KGeom *G
 static void choose_R(int kind, int Nu, int cmax, int *R, int *npt)
 {
     int best = 1; double bestscore = -1.0;
-    for (int r = 1; r <= cmax && Nu * r <= 256; ++r) {
+    for (int r = 1; r <= cmax && Nu * r <= (Nu > 256 ? MAXNU : 256); ++r) {
         const int n = (cmax + r - 1) / r;
         if (n > 16) continue;
         const int T = (Nu * r + 31) / 32 * 32;
@@ -180,7 +181,7 @@ struct Layout {
 };
 static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
 {
-    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > 256 || vg->Nv < 1 || vg->Nv > MAXCHUNK) return 1;
+    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > MAXNU || vg->Nv < 1 || vg->Nv > MAXCHUNK) return 1;
     const size_t cells = (size_t)m->I * m->J, N = (size_t)vg->Nu * vg->Nv;
     const size_t Npad = (N + 15) & ~(size_t)15;
     const size_t nfx = (size_t)(m->I + 1) * m->J, nfy = (size_t)m->I * (m->J + 1);
@@ -227,7 +228,7 @@ static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
 static const char *check_geometry(int kind, const UgksParams &T, const KGeom &G)
 {
     if (G.nchunk() < 1 || G.nchunk() > MAXCHUNK) return "bad chunk count";
-    if (G.npt < 1 || G.npt > 16 || G.R < 1 || T.Nu * G.R > 256 || G.R * G.npt < G.cmax) return "R / points per thread out of range";
+    if (G.npt < 1 || G.npt > 16 || G.R < 1 || T.Nu * G.R > (T.Nu > 256 ? MAXNU : 256) || G.R * G.npt < G.cmax) return "R / points per thread out of range";
     if (G.strip < 0 || G.strip > T.I) return "strip out of range (0 = automatic, else 1..I)";
     if (jit_smem(kind, T, G) > 227 * 1024) return "chunk does not fit in shared memory";
     return nullptr;
@@ -320,7 +321,7 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     *out = nullptr;
     if (!m || !vg || !gas || !bcs || !workspace_dev) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     Layout L;
-    if (make_layout(m, vg, &L)) return fail(c, UGKS_EINVAL, "%s", "invalid mesh or velocity grid size (I,J >= 2; 1 <= Nu <= 256)");
+    if (make_layout(m, vg, &L)) return fail(c, UGKS_EINVAL, "%s", "invalid mesh or velocity grid size (I,J >= 2; 1 <= Nu <= 512)");
     if (!(m->x1 > m->x0) || !(m->y1 > m->y0)) return fail(c, UGKS_EINVAL, "%s", "empty domain");
     if (!vg->u || !vg->wu || !vg->v || !vg->wv) return fail(c, UGKS_EINVAL, "%s", "NULL velocity arrays");
     if (gas->Pr != 1.0) return fail(c, UGKS_EINVAL, "%s", "Pr must be 1 (BGK)");
@@ -460,7 +461,7 @@ int ugks_set_option(ugks_ctx *c, const char *name, int value)
                 KGeom G = kind == JIT_MOMENTS ? *c->gm : *c->gu;
                 if (!strcmp(base, "strip")) { if (value < 0 || value > P.I) return fail(c, UGKS_EINVAL, "%s", "strip out of range"); G.strip = value; }
                 else if (!strcmp(base, "R")) {
-                    if (value < 1 || P.Nu * value > 256) return fail(c, UGKS_EINVAL, "%s", "R out of range");
+                    if (value < 1 || P.Nu * value > (P.Nu > 256 ? MAXNU : 256)) return fail(c, UGKS_EINVAL, "%s", "R out of range");
                     G.R = value; G.npt = (G.cmax + value - 1) / value; G.strip = 0;
                 } else {                                             // re-chunk with at most `value` rows per chunk
                     if (value < 1 || value > 56) return fail(c, UGKS_EINVAL, "%s", "chunk rows out of range");

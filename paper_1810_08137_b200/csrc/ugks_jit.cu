@@ -32,6 +32,7 @@ int cdivi(int a, int b) { return (a + b - 1) / b; }
 int nsxm() { const char *e = getenv("UGKS_NSXM"); const int n = e ? atoi(e) : 3; return n < 2 ? 2 : (n > 4 ? 4 : n); }   // x-ring slots of k_cell_moments
 int smem_mom_q(const UgksParams &P, const KGeom &G, bool mixed, int QB);
 int smem_upd_q(const UgksParams &P, const KGeom &G, int ny, int QB);
+bool upd_slice(const UgksParams &P, const KGeom &G);
 int upd_rows(const UgksParams &P, const KGeom &G) { return G.nmix > 0 ? 4 : (P.tangential ? 6 : 3); }
 // slot size of a staged chunk: MC*NU + 1 doubles rounded up to even, or to a 128-byte multiple if no resident CTA is lost to it
 int qb_of(int kind, const UgksParams &P, const KGeom &G)
@@ -58,9 +59,19 @@ int smem_mom_q(const UgksParams &P, const KGeom &G, bool mixed, int QB)
     return total * 8;
 }
 int smem_upd(const UgksParams &P, const KGeom &G, int ny) { return smem_upd_q(P, G, ny, qb_of(JIT_UPDATE, P, G)); }
+// k_flux_update stages, of the v-tables of a face / cell record, only the rows of its chunk when that saves at least 64 doubles
+// per table (SLICE in ugks_jit_update.cuh; developer override UGKS_SLICE=0/1)
+bool upd_slice(const UgksParams &P, const KGeom &G)
+{
+    if (const char *e = getenv("UGKS_SLICE")) return atoi(e) != 0;
+    return P.NvP - pad2i(G.cmax + 1) >= 64;
+}
 int smem_upd_q(const UgksParams &P, const KGeom &G, int ny, int QB)
 {
-    const int size = ny * QB + 3 * P.frs + P.crs;
+    const bool sl = upd_slice(P, G);
+    const int msl = pad2i(G.cmax + 1);
+    const int frs = sl ? FR_NCOEF + P.NuP + msl : P.frs, crs = sl ? CR_NCOEF + 2 * P.NuP + 2 * msl : P.crs;
+    const int size = ny * QB + 3 * frs + crs;
     return (3 * QB + 2 * size) * 8 + 5 * 8;
 }
 // CTAs per SM for __launch_bounds__: what shared memory allows, capped so that a thread keeps at least `regs` registers
@@ -132,7 +143,7 @@ std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const dou
         DEF("G_MINB_MOM", min_blocks(threads, sm_u, 128)); DEF("G_MINB_MOMX", min_blocks(threads, sm_m, 128));
     } else {
         const int su3 = smem_upd(P, G, P.tangential ? 6 : 3), su4 = smem_upd(P, G, 4);
-        DEF("G_SMEM_UPD3", su3); DEF("G_SMEM_UPD4", su4);
+        DEF("G_SMEM_UPD3", su3); DEF("G_SMEM_UPD4", su4); DEF("G_SLICE", upd_slice(P, G) ? 1 : 0);
         DEF("G_MINB_UPD", min_blocks(threads, G.nmix > 0 ? su4 : su3, 128));
     }
 #undef DEF

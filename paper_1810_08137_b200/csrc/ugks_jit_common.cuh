@@ -157,21 +157,28 @@ struct false_c { static constexpr bool value = false; };
 // ---- limiter ----------------------------------------------------------------------------------------------------------
 // h*sigma of the van Leer limiter (AMB-4) from un-normalised differences dm = f_c - f_{c-1}, dp = f_{c+1} - f_c:
 //   h*sigma = (Delta/2) * 2 (dm/Delta)(dp/Delta)/((dm+dp)/Delta) = dm dp / (dm + dp)   if dm dp > 0, else 0.
-// The reciprocal is MUFU.RCP64H (rel. error 2^-23) refined by one cubic step r (1 + e + e^2), e = 1 - s r: error e^3 ~ 2^-69,
-// i.e. r is within ~1 ulp.  The sign test reads the high word: a product that underflowed to a denormal counts as 0, as in
+// The reciprocal is MUFU.RCP64H (rel. error 2^-23) refined by one cubic step (1 + e + e^2), e = 1 - s r: error e^3 ~ 2^-69,
+// applied to the quotient q0 = pr r: hs = q0 (1 + e + e^2) is within ~1 ulp of pr / s.  The sign test reads the high word: a product that underflowed to a denormal counts as 0, as in
 // AMB-4's "underflow gives sigma = 0".
 __device__ __forceinline__ double vl_half(double dm, double dp)
 {
     const double pr = dm * dp, s = dm + dp;
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));
+#if defined(UGKS_VL_SERIAL)                                          // round-2 form: refine r, then multiply (one level deeper)
     const double e = fma(-s, r, 1.0);
-#ifdef UGKS_VL_NEWTON2                                               // experiment: quadratic step, error e^2 ~ 2^-46
-    r = fma(r, e, r);
-#else
     const double t = fma(e, e, e);
     r = fma(r, t, r);
-#endif
     const double hs = pr * r;
+#elif defined(UGKS_VL_NEWTON2)                                       // experiment: one Newton step on the quotient, error ~ 2^-46
+    const double q0 = pr * r;
+    const double hs = fma(fma(-s, q0, pr), r, q0);
+#else
+    // q0 = pr r0 is formed beside e = 1 - s r0, so the chain after s is MUFU, e, t = e + e^2, q0 (1 + t): four deep, not five
+    const double q0 = pr * r;
+    const double e = fma(-s, r, 1.0);
+    const double t = fma(e, e, e);
+    const double hs = fma(q0, t, q0);
+#endif
     return __double2hiint(pr) > 0 ? hs : 0.0;
 }

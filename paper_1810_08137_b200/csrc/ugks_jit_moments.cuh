@@ -98,7 +98,7 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
     double *part = sm + L::O_PART;                                   // [NA][BT]
     double *col = sm + L::O_COL;                                     // [2][NC][NUS]
     double *fac = sm + L::O_FAC;                                     // [NFAC][NUS]
-    double *mtab = sm + L::O_MTAB;                                   // [NROW][6]: w, w v, w v^2, w v^3, w v^4, H(v)
+    double *mtab = sm + L::O_MTAB;                                   // [NROW][6]: w, w v, w v^2, w v^3, w v^4, H(v) / weight of A_0
     double *ires = sm + L::O_IRES;                                   // [2][NITEM] stage-3 item results
     uint64_t *bars = reinterpret_cast<uint64_t *>(sm + L::O_BARS);   // [NSXM] x rows, [2] y stages, [1] part free
 

@@ -25,15 +25,23 @@
 #include "ugks_jit_common.cuh"
 
 constexpr int NSX = 3;                                               // x-ring slots: rows a, a+1 live, a+2 in flight
+// Record slices: a chunk needs, of the separable factors over v (E_m[Nv] of a face record, g_v^n[Nv], g_v^{n+1}[Nv] of a cell record),
+// only its own rows.  With SLICE the stage holds [coefficients | factors over u | rows m0a .. m0a + MSL) of the factors over v]
+// (m0a = m0 rounded down to even: bulk copies start 16-byte aligned), two / three bulk copies per record instead of one: on wide
+// velocity grids (C5: 5 of 200 rows per chunk) the whole records are twice the bytes of the chunk's f rows.
+constexpr bool SLICE = G_SLICE != 0;
+constexpr int MSL = pad2c(MC + 1);                                   // staged rows of a factor table over v
+constexpr int FRSS = SLICE ? FR_NCOEF + NUP + MSL : FRS, CRSS = SLICE ? CR_NCOEF + 2 * NUP + 2 * MSL : CRS;
+constexpr int VTS = SLICE ? MSL : NVP;                               // stride between the two v-tables of a staged cell record
 
 template <int NY>
 struct StageL {                                                      // offsets in doubles inside one step stage
     static constexpr int yrow = 0;
     static constexpr int xrec = yrow + NY * QB;
-    static constexpr int ylrec = xrec + FRS;
-    static constexpr int yurec = ylrec + FRS;
-    static constexpr int crec = yurec + FRS;
-    static constexpr int size = crec + CRS;
+    static constexpr int ylrec = xrec + FRSS;
+    static constexpr int yurec = ylrec + FRSS;
+    static constexpr int crec = yurec + FRSS;
+    static constexpr int size = crec + CRSS;
     static constexpr int BYTES = (NSX * QB + 2 * size) * 8 + (NSX + 2) * 8;
 };
 
@@ -49,7 +57,25 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     const int m0 = ch.x, mc = ch.y;
     const int q0 = m0 * NU, qa = q0 & ~1, qsh = q0 - qa;
     const uint32_t bytes = (uint32_t)(pad2c(mc * NU + qsh) * 8);
-    constexpr uint32_t fbytes = FRS * 8, cbytes = CRS * 8;
+    const int m0a = m0 & ~1, msh = m0 - m0a;                         // SLICE: first staged row of the v-tables, shift of the chunk inside
+    const uint32_t sbytes = (uint32_t)(pad2c(mc + msh) * 8);
+    const uint32_t fbytes = SLICE ? (FR_NCOEF + NUP) * 8 + sbytes : FRS * 8, cbytes = SLICE ? (CR_NCOEF + 2 * NUP) * 8 + 2 * sbytes : CRS * 8;
+    // whole record, or its head and the chunk's rows of its v-tables
+    auto copy_frec = [&](double *dst, const double *src, uint64_t *bar) {
+        if constexpr (!SLICE) tma_load_1d(dst, src, FRS * 8, bar);
+        else {
+            tma_load_1d(dst, src, (FR_NCOEF + NUP) * 8, bar);
+            tma_load_1d(dst + FR_NCOEF + NUP, src + FR_NCOEF + NUP + m0a, sbytes, bar);
+        }
+    };
+    auto copy_crec = [&](double *dst, const double *src, uint64_t *bar) {
+        if constexpr (!SLICE) tma_load_1d(dst, src, CRS * 8, bar);
+        else {
+            tma_load_1d(dst, src, (CR_NCOEF + 2 * NUP) * 8, bar);
+            tma_load_1d(dst + CR_NCOEF + 2 * NUP, src + CR_NCOEF + 2 * NUP + m0a, sbytes, bar);
+            tma_load_1d(dst + CR_NCOEF + 2 * NUP + MSL, src + CR_NCOEF + 2 * NUP + NVP + m0a, sbytes, bar);
+        }
+    };
 
     double *ring = reinterpret_cast<double *>(smem_raw);             // [NSX][QB]
     double *stages = ring + NSX * QB;                                // [2][L::size]
@@ -79,7 +105,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
             constexpr int JN = SGN > 0 ? -1 : 1, JO = -JN;
             const int c = st - 1;
             mbar_expect_tx(bar, fbytes + 6 * bytes + (have_cell ? 2 * fbytes + cbytes : 0));
-            tma_load_1d(S + L::xrec, A.frec0 + ((size_t)j * (GI + 1) + st) * FRS, fbytes, bar);
+            copy_frec(S + L::xrec, A.frec0 + ((size_t)j * (GI + 1) + st) * FRS, bar);
             tma_load_1d(S + L::yrow, cell_row_ptr(fcur, A.ghost, c, j + DJ0) + qa, bytes, bar);
             tma_load_1d(S + L::yrow + QB, cell_row_ptr(fcur, A.ghost, c, j + DJ1) + qa, bytes, bar);
             tma_load_1d(S + L::yrow + 2 * QB, cell_row_ptr(fcur, A.ghost, c, j + DJ2) + qa, bytes, bar);
@@ -88,14 +114,14 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
             tma_load_1d(S + L::yrow + 5 * QB, cell_row_ptr(fcur, A.ghost, c + 1, j + JO) + qa, bytes, bar);
             if (have_cell) {
                 const double *yl = A.frec1 + ((size_t)j * GI + c) * FRS;
-                tma_load_1d(S + L::ylrec, yl, fbytes, bar);
-                tma_load_1d(S + L::yurec, yl + (size_t)GI * FRS, fbytes, bar);
-                tma_load_1d(S + L::crec, A.crec + ((size_t)j * GI + c) * CRS, cbytes, bar);
+                copy_frec(S + L::ylrec, yl, bar);
+                copy_frec(S + L::yurec, yl + (size_t)GI * FRS, bar);
+                copy_crec(S + L::crec, A.crec + ((size_t)j * GI + c) * CRS, bar);
             }
             return;
         }
         mbar_expect_tx(bar, fbytes + (have_cell ? NY * bytes + 2 * fbytes + cbytes : 0));
-        tma_load_1d(S + L::xrec, A.frec0 + ((size_t)j * (GI + 1) + st) * FRS, fbytes, bar);
+        copy_frec(S + L::xrec, A.frec0 + ((size_t)j * (GI + 1) + st) * FRS, bar);
         if (have_cell) {
             const size_t cell = st - 1;
             int yst;
@@ -110,9 +136,9 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
                 tma_load_1d(S + L::yrow + 3 * QB, y3p + cell * yst, bytes, bar);
             }
             const double *yl = A.frec1 + ((size_t)j * GI + cell) * FRS;
-            tma_load_1d(S + L::ylrec, yl, fbytes, bar);
-            tma_load_1d(S + L::yurec, yl + (size_t)GI * FRS, fbytes, bar);
-            tma_load_1d(S + L::crec, A.crec + ((size_t)j * GI + cell) * CRS, cbytes, bar);
+            copy_frec(S + L::ylrec, yl, bar);
+            copy_frec(S + L::yurec, yl + (size_t)GI * FRS, bar);
+            copy_crec(S + L::crec, A.crec + ((size_t)j * GI + cell) * CRS, bar);
         }
     };
     if (tid == 0) {
@@ -130,10 +156,11 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     // Per-thread points p: velocity row m = r + p R; byte offsets are thread base + immediates.  A point outside the chunk
     // (the last point when R*NPT > MC, the tail of a ragged chunk) re-reads the chunk's first element; only its store is masked.
     constexpr int QSTEP = R * NU * 8, MSTEP = R * 8;
-    const int qb0 = (qsh + r * NU + k) * 8, mb0 = (m0 + r) * 8;
+    const int mfirst = (SLICE ? msh : m0) * 8;                       // byte offset of the chunk's first row in a staged v-table
+    const int qb0 = (qsh + r * NU + k) * 8, mb0 = mfirst + r * 8;
     int qo[NPT], mo[NPT];
 #pragma unroll
-    for (int p = 0; p < NPT; ++p) { qo[p] = r + p * R < mc ? p * QSTEP : qsh * 8 - qb0; mo[p] = r + p * R < mc ? p * MSTEP : m0 * 8 - mb0; }
+    for (int p = 0; p < NPT; ++p) { qo[p] = r + p * R < mc ? p * QSTEP : qsh * 8 - qb0; mo[p] = r + p * R < mc ? p * MSTEP : mfirst - mb0; }
 #define QOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * QSTEP : qo[p])
 #define MOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * MSTEP : mo[p])
     double vn[NPT], fm[NPT], fc[NPT], Fprev[NPT];
@@ -175,15 +202,17 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
 #ifndef UGKS_UNROLL_U
 #define UGKS_UNROLL_U (STRIP >= 16 ? 2 : 1)                        // measured (C4): -7 % (the ring / stage parities and half of the register rotation fold away); short strips: +10 %
 #endif
-#pragma unroll UGKS_UNROLL_U
-    for (int a = c0; a <= c1; ++a) {                                 // x-face a, then cell a-1
+    // one step: x-face a, then cell a-1.  The first step of a march (a = c0) has no cell to finish: it is peeled off (HC = false) so
+    // that the steady-state body carries no "have a cell" branch between its points and the points of a thread form one basic block
+    // (the independent FP64 chains of the NPT points can then be interleaved by the scheduler)
+    auto step = [&](const int a, auto hc) {
+        constexpr bool have_cell = decltype(hc)::value;
         const unsigned char *S = stages_b + stage_i * (L::size * 8);
         mbar_wait(&bars[NSX + stage_i], stage_phase);
         if (stage_i) stage_phase ^= 1;
         stage_i ^= 1;
         mbar_wait(&bars[xw_slot], xw_phase);                         // row a+1
         if (++xw_slot == NSX) { xw_slot = 0; xw_phase ^= 1; }
-        const bool have_cell = a > c0;
         // ---- x-face a: polynomial column of this thread (n = u_k; cubic in t = v_m)
         const double *xr = reinterpret_cast<const double *>(S + L::xrec * 8);
         const double *xlr = xr + (posx ? FR_L : FR_R);
@@ -238,7 +267,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         const bool nb_ghost = TG && (SGN > 0 ? (j - 1 < 0 && BCY0 == BC_FIXED) : (j + 1 >= GJ && BCY1 == BC_FIXED));
         const bool tgb = TG && (a < 2 || a + 2 > GI || j < 1 || j > GJ - 2);      // near a boundary: take the flagged body
         const unsigned char *ylm = S + (L::ylrec + FR_NCOEF + NUP) * 8 + mb0, *yum = S + (L::yurec + FR_NCOEF + NUP) * 8 + mb0;
-        const unsigned char *cgn = S + (L::crec + CR_NCOEF + 2 * NUP) * 8 + mb0, *cgp = cgn + NVP * 8;
+        const unsigned char *cgn = S + (L::crec + CR_NCOEF + 2 * NUP) * 8 + mb0, *cgp = cgn + VTS * 8;
         unsigned char *out = out_row + (size_t)max(a - 1, 0) * (NPAD * 8);
 
         auto body = [&](auto fl) {                                   // fl: some stencil of this step touches a wall
@@ -270,7 +299,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
                 Fprev[p] = F;
                 const double own = posx ? fc[p] : fm[p];             // row of cell a-1
                 fm[p] = fc[p]; fc[p] = fn;
-                if (!have_cell) continue;
+                if constexpr (!have_cell) continue;
                 // y-faces of cell a-1: G = F / n
                 const double n = t;
                 const bool pos = SGN > 0 || (SGN == 0 && n > 0.0);
@@ -322,7 +351,10 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         }
         issuer += 32;
         if (issuer >= BT) issuer = 0;
-    }
+    };
+    step(c0, false_c{});
+#pragma unroll UGKS_UNROLL_U
+    for (int a = c0 + 1; a <= c1; ++a) step(a, true_c{});
 }
 
 static_assert(StageL<TG ? 6 : 3>::BYTES == G_SMEM_UPD3 && StageL<4>::BYTES == G_SMEM_UPD4, "host mirror of the shared-memory layout (ugks_jit.cu) disagrees");
@@ -339,8 +371,21 @@ static_assert(!TG, "the tangential reconstruction needs sorted velocity nodes (n
 extern "C" __global__ void __launch_bounds__(BT, G_MINB_UPD) k_flux_update(const KArgs A, const int chunk0)
 {
     int b = blockIdx.x;
+#ifndef UGKS_ORDER_U
+#define UGKS_ORDER_U 0
+#endif
+#if UGKS_ORDER_U == 1
+    // launch order: chunks fastest, then rows, then strips -- the CTAs that read the face and cell records of a cell (one per chunk)
+    // run together, so the records cross HBM once per step, and so do the y-neighbour rows (rows j-2 .. j+2 are in flight together)
+    const int c = b % NCHUNK; b /= NCHUNK;
+    const int j = b % GJ, s = b / GJ;
+#elif UGKS_ORDER_U == 2
     const int j = b % GJ; b /= GJ;
-    const int s = b % NSTRIP, c = b / NSTRIP;                        // launch order: rows fastest, then strips, then chunks
+    const int c = b % NCHUNK, s = b / NCHUNK;
+#else
+    const int j = b % GJ; b /= GJ;
+    const int s = b % NSTRIP, c = b / NSTRIP;                        // rows fastest, then strips, then chunks
+#endif
     const int4 ch = c_chunks[chunk0 + c];
     if (ch.z > 0) flux_update_body<1>(A, ch, j, s);
     else if (ch.z < 0) flux_update_body<-1>(A, ch, j, s);

@@ -81,6 +81,18 @@ def test_stale_shared_memory_is_never_read(name, I, J, nuv):
     _check(_run_pair(workloads.channel_config(name, I=I, J=J, Nuv=nuv), 3, options=(("poison", 1),)), 3 * TOL_1)
 
 
+@pytest.mark.parametrize("nu,nv,I,J", [(320, 12, 6, 5), (321, 9, 5, 4), (512, 8, 4, 3)])
+def test_more_than_256_velocity_columns(nu, nv, I, J):
+    """Nu > 256: a CTA of Nu threads, one per column (R = 1), up to 512 columns; even, odd (u = 0 column) and the
+    largest width, C5's wide-velocity physics on [-20,20] x [-20,20], shared memory poisoned, three steps."""
+    import dataclasses
+    p = workloads.channel_config("C5", I=I, J=J)
+    u, wu = workloads.trapezoid_grid(nu, 20.0)
+    v, wv = workloads.trapezoid_grid(nv, 20.0)
+    p = dataclasses.replace(p, u=u, wu=wu, v=v, wv=wv, name=f"C5-{nu}x{nv}")
+    _check(_run_pair(p, 3, options=(("poison", 1),)), 3 * TOL_1)
+
+
 TG = (("tangential", 1),)
 
 

@@ -58,8 +58,10 @@ def _cpu_model():
 
 
 def fp64_peak_measured():
-    """thread-level DFMA/s of the plain FP64 pipe, measured by bench_fp64_peak.cu (compiled here with nvcc for sm_100a; a
-    bench-side helper library, not part of libugks)."""
+    """(pipe rate, three-operand rate): thread-level DFMA/s of the plain FP64 pipe measured by bench_fp64_peak.cu (compiled here
+    with nvcc for sm_100a; a bench-side helper library, not part of libugks) -- with two of the three operands reused (the rate
+    of the 16-lane pipe itself: the roofline peak) and with three distinct register operands per DFMA (what register-operand
+    fetch allows a kernel whose operands all differ; reported beside the peak, not used as the denominator)."""
     import ctypes as C
     src, so = os.path.join(ROOT, "bench_fp64_peak.cu"), os.path.join(ROOT, "libbench_fp64.so")
     if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(src):
@@ -68,11 +70,11 @@ def fp64_peak_measured():
         subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-Xcompiler", "-fPIC", "-shared", "-o", tmp, src], check=True)
         os.replace(tmp, so)
     lib = C.CDLL(so)
-    out = C.c_double(0.0)
-    rc = lib.bench_fp64_peak(C.byref(out))
+    out, out3 = C.c_double(0.0), C.c_double(0.0)
+    rc = lib.bench_fp64_peak(C.byref(out)) or lib.bench_fp64_peak_3op(C.byref(out3))
     if rc:
         raise RuntimeError(f"bench_fp64_peak -> {rc}")
-    return float(out.value)
+    return float(out.value), float(out3.value)
 
 
 def _peaks():
@@ -291,7 +293,7 @@ def main():
         return res
 
     p = workloads.channel_config(args.config)
-    fp64_measured = fp64_peak_measured()
+    fp64_measured, fp64_3op = fp64_peak_measured()
 
     def hbm_fracs(q, ms_step, kernel_ms):
         """HBM-roofline fractions of a workload: per f-sized kernel (its algorithmic bytes / its time) and for the step against
@@ -315,6 +317,7 @@ def main():
             t = kernel_ms[k] * 1e-3
             out[k] = {"fp64_inst_per_point": c["fp64_thread_inst"] / q.points, "inst_per_point": c["thread_inst"] / q.points,
                       "fp64_inst_per_s": c["fp64_thread_inst"] / t, "frac_of_fp64_peak": c["fp64_thread_inst"] / t / fp64_measured,
+                      "frac_of_3operand_dfma_rate": c["fp64_thread_inst"] / t / fp64_3op,
                       "dram_bytes": c.get("dram_bytes")}
         return out
 
@@ -333,6 +336,9 @@ def main():
         roof = {"bound": "alu", "kernel": dom, "achieved": alu[dom]["fp64_inst_per_s"] / 1e12, "peak": fp64_measured / 1e12,
                 "unit": "T FP64 thread-inst/s", "frac": alu[dom]["frac_of_fp64_peak"], "traffic": alu[dom]["dram_bytes"],
                 "peak_source": "measured here: bench_fp64_peak.cu, 8 independent DFMA chains per thread (nominal 148 SMs x 4 x 16 lanes x 1.965 GHz = %.3g)" % FP64_PEAK,
+                "peak_3operand": fp64_3op / 1e12, "frac_of_3operand": alu[dom]["fp64_inst_per_s"] / fp64_3op,
+                "peak_3operand_source": "measured here: 32 accumulators, x[i] += x[i+5] * x[i+11] (three distinct register operands per DFMA): the rate "
+                                        "register-operand fetch allows; context for frac, not its denominator",
                 "counts_source": "profiles/r2_counts.json (ncu --set full of this build, static per build; times are live)"}
     else:
         roof = {"bound": "hbm", "kernel": dom, "achieved": hbm[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",

@@ -141,6 +141,7 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
             pw *= u;
         }
     }
+    for (int i = tid; i < L::O_FAC - L::O_COL; i += BT) col[i] = 0.0;   // stage 3 may read (times a zero factor) entries no cell has written yet
     for (int i = tid; i < NROW; i += BT) {
         const bool in = i < mc;
         const double v = in ? c_v[m0 + i] : 0.0, w = in ? c_wv[m0 + i] : 0.0;
@@ -195,6 +196,21 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
         }
     }
     __syncthreads();
+    // the factors of a thread's stage-3 items never change along the march: short items keep them in registers (UGKS_S3REG doubles
+    // at most), which halves the shared-memory loads of stage 3 -- the loads with most of this kernel's bank conflicts
+#ifndef UGKS_S3REG
+#define UGKS_S3REG 32
+#endif
+    constexpr int S3LEN = cmaxi(L::PERX, L::PERY);
+    constexpr bool FREG = S3R * S3LEN <= UGKS_S3REG;
+    double itfac[FREG ? S3R * S3LEN : 1];
+    if constexpr (FREG) {
+#pragma unroll
+        for (int q = 0; q < S3R; ++q)
+#pragma unroll
+            for (int n = 0; n < S3LEN; ++n)
+                itfac[q * S3LEN + n] = n < it_n[q] ? ldsd(reinterpret_cast<const unsigned char *>(fac), it_f[q] + n * 8) : 0.0;
+    }
 
     // per-thread points: row m = r + p*R; byte offsets are thread base + immediates.  A point outside the chunk (the last
     // point when R*NPT > MC, the tail of a ragged chunk) re-reads the chunk's first element and carries a zero weight row
@@ -367,11 +383,23 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
             for (int q = 0; q < S3R; ++q) {
                 if (tid + q * BT < NITEM) {
                     constexpr int LEN = cmaxi(L::PERX, L::PERY);
-                    double sum = 0.0;
+                    double sum = 0.0, sum1 = 0.0;                    // two chains
+                    if constexpr (FREG) {
+                        // no range test per element: beyond the item's range the register factor is zero and the column entry read
+                        // instead is a finite number (a neighbouring column, a zeroed pad element or the factor table behind the buffer)
 #pragma unroll
-                    for (int n = 0; n < LEN; ++n)
-                        if (n < it_n[q]) sum = fma(ldsd(fb, it_f[q] + n * 8), ldsd(cc, it_c[q] + n * 8), sum);
-                    ires[(c3 & 1) * NITEM + tid + q * BT] = sum;
+                        for (int n = 0; n < LEN; n += 2) {
+                            sum = fma(itfac[q * S3LEN + n], ldsd(cc, it_c[q] + n * 8), sum);
+                            if (n + 1 < LEN) sum1 = fma(itfac[FREG ? q * S3LEN + n + 1 : 0], ldsd(cc, it_c[q] + (n + 1) * 8), sum1);
+                        }
+                    } else {
+#pragma unroll
+                        for (int n = 0; n < LEN; n += 2) {
+                            if (n < it_n[q]) sum = fma(ldsd(fb, it_f[q] + n * 8), ldsd(cc, it_c[q] + n * 8), sum);
+                            if (n + 1 < LEN && n + 1 < it_n[q]) sum1 = fma(ldsd(fb, it_f[q] + (n + 1) * 8), ldsd(cc, it_c[q] + (n + 1) * 8), sum1);
+                        }
+                    }
+                    ires[(c3 & 1) * NITEM + tid + q * BT] = sum + sum1;
                 }
             }
         }

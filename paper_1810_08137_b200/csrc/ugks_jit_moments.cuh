@@ -273,6 +273,7 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
             double acc[NA];
 #pragma unroll
             for (int i = 0; i < NA; ++i) acc[i] = 0.0;
+            double zfix = 0.0;                                       // ZROW: the half of the v = 0 row's weight that A_0 does not get
             auto pass = [&](auto fl) {
                 constexpr bool FL = decltype(fl)::value;
 #pragma unroll
@@ -292,14 +293,14 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
                     acc[3] = fma(w01.x, hx, acc[3]); acc[4] = fma(w01.y, hx, acc[4]); acc[5] = fma(w23.x, hx, acc[5]);
                     // y-faces: n = v_m;  A_a = sum wv n^a f0 (a = 0..3),  B_a = sum wv n^a h sigma (a = 2..4)
                     if constexpr (!MIXED) {
-                        const double f0 = fma(sy, hy, c);
-                        if (ZROW && p == 0) acc[NA - 1] = wz * (c - hy);    // v = 0 row (row 0 of the flagged chunk): y- half
-                        acc[6] = fma(w4h.y, f0, acc[6]); acc[7] = fma(w01.y, f0, acc[7]); acc[8] = fma(w23.x, f0, acc[8]);
-                        acc[9] = fma(w23.y, f0, acc[9]);
+                        // A_a = sum wv n^a (f_c + sy h sigma) = Cc_a + sy Hy_a: the sums of f_c (Cc_0..2 are the C_b above, Cc_3 in acc[9]) and of
+                        // h sigma_y (Hy_0, Hy_1 in acc[6], acc[7]; Hy_2..4 are the B_a) are kept apart and combined once per cell after
+                        // the point loop -- 12 accumulations per point instead of 13 and no f0 per point
+                        if (ZROW && p == 0) { acc[NA - 1] = wz * (c - hy); zfix = (w01.x - w4h.y) * fma(sy, hy, c); }   // v = 0 row: halves
+                        acc[6] = fma(w01.x, hy, acc[6]); acc[7] = fma(w01.y, hy, acc[7]); acc[9] = fma(w23.y, c, acc[9]);
                         acc[10] = fma(w23.x, hy, acc[10]); acc[11] = fma(w23.y, hy, acc[11]); acc[12] = fma(w4h.x, hy, acc[12]);
-                        if constexpr (TG) {                          // tangential slopes: D_b = sum wv v^b (h_y sigma_y), E_a = sum wv v^a (h_x sigma_x)
-                            acc[13] = fma(w01.y, hy, acc[13]); acc[14] = fma(w23.x, hy, acc[14]); acc[15] = fma(w23.y, hy, acc[15]);
-                            acc[16] = fma(w01.y, hx, acc[16]); acc[17] = fma(w23.x, hx, acc[17]); acc[18] = fma(w23.y, hx, acc[18]);
+                        if constexpr (TG) {                          // tangential slopes: D_b = Hy_b (b = 1..3) come for free; E_a = sum wv v^a (h_x sigma_x)
+                            acc[18] = fma(w23.y, hx, acc[18]);      // E_3 (E_1, E_2 are B_1, B_2 of the x-sums)
                         }
                     } else {                                         // AMB-5: H(0) = 1/2 sends half of the point to either side
                         const double hp = w4h.y, hm = 1.0 - hp, fp = (c + hy) * hp, fm = (c - hy) * hm, gp = hy * hp, gm = hy * hm;
@@ -314,6 +315,15 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
                 }
             };
             if (xm_miss || xp_miss || ym_miss || yp_miss) pass(true_c{}); else pass(false_c{});
+            if constexpr (!MIXED) {                                  // combine: acc[6..9] = A_0..3; TG: acc[13..15] = D_1..3, acc[16], acc[17] = E_1, E_2
+                const double hy0 = acc[6], hy1 = acc[7], c3 = acc[9];
+                if constexpr (TG) {
+                    acc[13] = hy1; acc[14] = acc[10]; acc[15] = acc[11];
+                    acc[16] = acc[4]; acc[17] = acc[5];
+                }
+                acc[6] = fma(sy, hy0, acc[0]) - zfix; acc[7] = fma(sy, hy1, acc[1]); acc[8] = fma(sy, acc[10], acc[2]);
+                acc[9] = fma(sy, acc[11], c3);
+            }
             if (R == 1) {                                            // the thread's sums are the column sums: stage 2 folded in
                 if (active) {
                     double *cc = col + (a & 1) * NC * NUS + k;

@@ -458,18 +458,21 @@ int launch_setup(const UgksParams &P, const double *bc_prims, double *ghost, dou
 // ---------------------------------------------------------------------------------------------
 // k_tables: every exponential of the step (S6 and the two cell equilibria of U2), once per face / cell and node:
 // exp(-lam ((u-U)^2 + (v-V)^2)) = E_k[k] E_m[m] on the tensor-product grid, so a face needs Nu + Nv exponentials, not Nu Nv.
-// One thread per SEGMENT of 8 consecutive entries of one table (a face Maxwellian, g^n of a cell, g^{n+1} of a cell) and
+// One thread per SEGMENT of TSEG consecutive entries of one table (a face Maxwellian, g^n of a cell, g^{n+1} of a cell) and
 // direction.  Where the nodes of that direction are equally spaced (P.hu / P.hv > 0, checked at init) the segment costs three
-// exponentials instead of eight: with x_i = x_s + i h,  E_{i+1} = E_i D_i,  D_{i+1} = D_i Q,  E_s = exp(-lam (x_s - c)^2),
-// D_s = exp(-lam h (2 (x_s - c) + h)),  Q = exp(-2 lam h^2); seven steps add at most ~30 roundings (3e-15 relative).  Segments in
+// exponentials instead of TSEG: with x_i = x_s + i h,  E_{i+1} = E_i D_i,  D_{i+1} = D_i Q,  E_s = exp(-lam (x_s - c)^2),
+// D_s = exp(-lam h (2 (x_s - c) + h)),  Q = exp(-2 lam h^2); seven steps add at most ~30 roundings (3e-15 relative; segments of 16 were
+// measured: no faster, and 1.3e-14 at the end of a segment breaks the fixed-point test's 1e-14).  Segments in
 // the far tail (E_s or D_s outside the normal range) and unequally spaced nodes take the direct exponentials.
-constexpr int TSEG = 8;
-__global__ void __launch_bounds__(256) k_tables(const UgksParams P)
+#ifndef UGKS_TSEG
+#define UGKS_TSEG 8
+#endif
+constexpr int TSEG = UGKS_TSEG;
+__global__ void __launch_bounds__(256) k_tables(const UgksParams P, const unsigned TPB)      // TPB: tables per block pass (about 256 / segments per table)
 {
     const unsigned nsu = (P.NuP + TSEG - 1) / TSEG, nsv = (P.NvP + TSEG - 1) / TSEG, nseg = nsu + nsv;
     const long nfx = nfaces_x(P), nfy = nfaces_y(P), ncell = (long)P.I * P.J;
     const long ntab = nfx + nfy + 2 * ncell;
-    constexpr unsigned TPB = 16;                                     // tables per block pass
     for (long rec0 = (long)blockIdx.x * TPB; rec0 < ntab; rec0 += (long)gridDim.x * TPB) {
         for (unsigned i = threadIdx.x; i < TPB * nseg; i += blockDim.x) {
             const unsigned rl = i / nseg, sg = i - rl * nseg;
@@ -528,9 +531,11 @@ __global__ void __launch_bounds__(256) k_tables(const UgksParams P)
 int launch_tables(const UgksParams &P, cudaStream_t st)
 {
     const long ntab = (long)nfaces_x(P) + nfaces_y(P) + 2L * P.I * P.J;
-    long blocks = (ntab + 15) / 16;
+    const unsigned nseg = (P.NuP + TSEG - 1) / TSEG + (P.NvP + TSEG - 1) / TSEG;
+    const unsigned tpb = (256 + nseg - 1) / nseg;                    // every thread of a block pass has a segment
+    long blocks = (ntab + tpb - 1) / tpb;
     if (blocks > 148L * 128) blocks = 148L * 128;
-    k_tables<<<(int)blocks, 256, 0, st>>>(P);
+    k_tables<<<(int)blocks, 256, 0, st>>>(P, tpb);
     return 1;
 }
 int launch_moments_of_f(const UgksParams &P, const double *f, double *Wf, cudaStream_t st)

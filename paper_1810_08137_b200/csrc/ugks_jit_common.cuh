@@ -173,12 +173,22 @@ __device__ __forceinline__ double vl_half(double dm, double dp)
 #elif defined(UGKS_VL_NEWTON2)                                       // experiment: one Newton step on the quotient, error ~ 2^-46
     const double q0 = pr * r;
     const double hs = fma(fma(-s, q0, pr), r, q0);
-#else
-    // q0 = pr r0 is formed beside e = 1 - s r0, so the chain after s is MUFU, e, t = e + e^2, q0 (1 + t): four deep, not five
+#elif defined(UGKS_VL_SELECT_RESULT)                                 // round-2 form: select the 64-bit result (two FSEL)
     const double q0 = pr * r;
     const double e = fma(-s, r, 1.0);
     const double t = fma(e, e, e);
     const double hs = fma(q0, t, q0);
+#else
+    // q0 = pr r0 is formed beside e = 1 - s r0, so the chain after s is MUFU, e, t = e + e^2, q0 (1 + t): four deep, not five.
+    // The sign test acts on the seed: its low word is zero by construction (MUFU.RCP64H), so "no slope" is one 32-bit select of
+    // the high word; with r0 = 0 the chain gives q0 = 0, e = 1, t = 2, hs = fma(0, 2, 0) = 0 exactly.
+    r = __hiloint2double(__double2hiint(pr) > 0 ? __double2hiint(r) : 0, 0);
+    const double q0 = pr * r;
+    const double e = fma(-s, r, 1.0);
+    const double t = fma(e, e, e);
+    return fma(q0, t, q0);
 #endif
+#if defined(UGKS_VL_SERIAL) || defined(UGKS_VL_NEWTON2) || defined(UGKS_VL_SELECT_RESULT)
     return __double2hiint(pr) > 0 ? hs : 0.0;
+#endif
 }

@@ -48,6 +48,12 @@ def test_version_and_workspace_bytes(libugks):
     assert binding.workspace_bytes(p4) < 17e9                                # C4: 13.4 GB of f + 2.5 GB of per-face / per-cell records
     bad = workloads.channel_config("C1", I=1)
     assert binding.workspace_bytes(bad) == 0
+    # velocity grids: up to 512 columns (one thread per column of a CTA), not more
+    import dataclasses
+    for nu, ok in ((256, True), (512, True), (513, False)):
+        u, wu = workloads.trapezoid_grid(nu, 20.0)
+        q = dataclasses.replace(workloads.channel_config("C1"), u=u, wu=wu)
+        assert (binding.workspace_bytes(q) > 0) == ok, nu
 
 
 def test_argument_validation_happens_before_cuda(libugks):

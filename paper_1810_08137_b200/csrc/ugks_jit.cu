@@ -168,6 +168,8 @@ int jit_compile(int kind, const std::string &prelude, std::vector<char> *cubin, 
     const std::string inc = "--include-path=" + dir;
     std::vector<const char *> opts = { "--gpu-architecture=sm_100a", "-lineinfo", "--std=c++17", "-default-device", inc.c_str() };
     if (verbose) opts.push_back("--ptxas-options=-v");
+    std::string maxreg;
+    if (const char *e = getenv("UGKS_JIT_MAXREG")) { maxreg = std::string("--maxrregcount=") + e; opts.push_back(maxreg.c_str()); }   // developer aid
     const nvrtcResult rc = nvrtcCompileProgram(prog, (int)opts.size(), opts.data());
     size_t n = 0;
     nvrtcGetProgramLogSize(prog, &n);

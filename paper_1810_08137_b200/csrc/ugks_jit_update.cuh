@@ -200,7 +200,8 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     int stage_i = 0, stage_phase = 0;
     int issuer = 0;                                                  // thread that issues the bulk copies after this step (lane 0 of a rotating warp)
 #ifndef UGKS_UNROLL_U
-#define UGKS_UNROLL_U (STRIP >= 16 ? 2 : 1)                        // measured (C4): -7 % (the ring / stage parities and half of the register rotation fold away); short strips: +10 %
+#define UGKS_UNROLL_U ((STRIP >= 16 && NU * R >= 128) ? 2 : 1)     // measured: C4 (160 threads) -10 % (the ring / stage parities and half of the register
+                                                                     // rotation fold away), C5 0; CTAs of 64-96 threads (C3, M4-69) +3 %, short strips +10 %
 #endif
     // one step: x-face a, then cell a-1.  The first step of a march (a = c0) has no cell to finish: it is peeled off (HC = false) so
     // that the steady-state body carries no "have a cell" branch between its points and the points of a thread form one basic block

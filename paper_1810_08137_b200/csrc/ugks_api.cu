@@ -265,6 +265,10 @@ static int apply_geometry(ugks_ctx *c, int kind, const KGeom &G)
                 kind == JIT_MOMENTS ? "k_cell_moments" : "k_flux_update", G.nchunk(), G.cmax, G.R, G.npt, G2.strip, jit_ctas_per_sm(jk), jk->threads,
                 jit_smem(kind, T, G));
     if (kind == JIT_MOMENTS) {
+        // the moment buffer is laid out per chunk, and k_face_scalars reads entries that k_cell_moments never writes (of the y- set
+        // of the chunk that holds a v = 0 row only M00, M01, M02 are stored; the T sums without option "tangential"): they must be
+        // zero, so a new chunking starts from a zeroed buffer, as ugks_init does
+        CK(cudaMemsetAsync(c->P.cmom, 0, c->cells * (size_t)c->nchunk_alloc * CMS * 8, c->st), "apply_geometry");
         CK(cudaMemcpy(c->chunks_dev, G.chunks.data(), sizeof(int4) * G.nchunk(), cudaMemcpyHostToDevice), "apply_geometry");
         T.nchunk = G.nchunk(); T.nneg = G.nneg; T.npos = G.npos; T.nmix = G.nmix; T.cmax = G.cmax; T.R = G.R; T.npt = G.npt; T.strip = G2.strip;
         c->P = T;

@@ -81,6 +81,27 @@ def test_stale_shared_memory_is_never_read(name, I, J, nuv):
     _check(_run_pair(workloads.channel_config(name, I=I, J=J, Nuv=nuv), 3, options=(("poison", 1),)), 3 * TOL_1)
 
 
+def test_rechunking_a_live_context_on_an_odd_grid():
+    """The moment buffer is laid out per chunk and k_face_scalars reads entries k_cell_moments never writes (of the y- set of the chunk
+    that holds the v = 0 row only three sums are stored): a new chunking of a context that has already stepped must start from a
+    zeroed buffer.  One context, geometry options changed between steps (other chunkings -- the moment buffer only holds chunkings no finer than the default -- and other R),
+    against the oracle."""
+    from oracle import Oracle
+    from paper_1810_08137_b200 import Ugks
+    p = workloads.channel_config("C2", I=36, J=5, Nuv=69)
+    W, f, _ = workloads.initial_state(p)
+    o = Oracle(p, threads=8)
+    o.set_state(W, f)
+    g = Ugks(p)
+    g.set_state(W, f)
+    g.step(1); o.step(1)
+    for n, (name, value) in enumerate([("chunk_m_m", 35), ("chunk_m_m", 17), ("R_m", 2), ("chunk_m_m", 12), ("chunk_u", 7), ("chunk_m_m", 35)]):
+        g.set_option(name, value)
+        g.step(1); o.step(1)
+        r = _compare(g, o)
+        assert r["ef"] <= (n + 2) * TOL_1 and r["eW"] <= (n + 2) * TOL_1, (name, value, r["ef"], r["eW"])
+
+
 @pytest.mark.parametrize("nu,nv,I,J", [(320, 12, 6, 5), (321, 9, 5, 4), (512, 8, 4, 3)])
 def test_more_than_256_velocity_columns(nu, nv, I, J):
     """Nu > 256: a CTA of Nu threads, one per column (R = 1), up to 512 columns; even, odd (u = 0 column) and the

@@ -81,6 +81,68 @@ def test_stale_shared_memory_is_never_read(name, I, J, nuv):
     _check(_run_pair(workloads.channel_config(name, I=I, J=J, Nuv=nuv), 3, options=(("poison", 1),)), 3 * TOL_1)
 
 
+def _random_problem(rng):
+    """a random small problem: mesh, velocity grids (even / odd, narrow / wider than 256 columns), boundary types per side, Kn"""
+    I, J = int(rng.integers(2, 41)), int(rng.integers(2, 13))
+    Nu, Nv = int(rng.integers(3, 71)), int(rng.integers(3, 71))
+    if rng.random() < 0.15:
+        Nu, Nv, I, J = int(rng.integers(257, 400)), int(rng.integers(3, 12)), min(I, 8), min(J, 5)
+    u, wu = workloads.trapezoid_grid(Nu, float(rng.uniform(4, 8)))
+    v, wv = workloads.trapezoid_grid(Nv, float(rng.uniform(4, 8)))
+
+    def sides():
+        k = int(rng.integers(0, 4))
+        fixed = lambda rho: (workloads.BC_FIXED, rho, float(rng.uniform(-.1, .1)), float(rng.uniform(-.1, .1)), float(rng.uniform(.9, 1.1)))
+        wall = lambda: (workloads.BC_WALL, 1.0, float(rng.uniform(-.2, .2)), float(rng.uniform(-.2, .2)), float(rng.uniform(.9, 1.2)))
+        if k == 0:
+            return [(workloads.BC_PERIODIC, 1, 0, 0, 1)] * 2
+        if k == 1:
+            return [fixed(1.0), fixed(0.85)]
+        if k == 2:
+            return [wall(), wall()]
+        return [fixed(1.0), wall()] if rng.random() < 0.5 else [wall(), fixed(0.9)]
+
+    return workloads.Problem(I=I, J=J, x0=0.0, x1=float(rng.uniform(.5, 2)), y0=0.0, y1=float(rng.uniform(.5, 2)), u=u, wu=wu, v=v, wv=wv,
+                             Kn=float(10 ** rng.uniform(-3, 1)), bcs=sides() + sides(), cfl=float(rng.uniform(.3, .9)),
+                             seed=int(rng.integers(1, 1 << 30)), eps=(0.05, 0.05, 0.05, 0.05), rho_drop=0.0, name="random")
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_small_problems(seed):
+    """Seeded random problems (sizes, grids, boundary types per side, Kn over four decades, CFL), with and without the tangential
+    slopes, random strip lengths, shared memory poisoned; after the first steps the launch geometry of both kernels is changed on
+    the live context (other chunkings, R, strips: whatever the library accepts) and the run goes on.  GPU vs oracle, every step's bar."""
+    from oracle import Oracle
+    from paper_1810_08137_b200 import Ugks, UgksError
+    rng = np.random.default_rng(1810_08137 + seed)
+    p = _random_problem(rng)
+    tg = bool(rng.random() < 0.4)
+    W, f, _ = workloads.initial_state(p)
+    o = Oracle(p, threads=8, tangential=tg)
+    o.set_state(W, f)
+    g = Ugks(p)
+    g.set_option("poison", 1)
+    if tg:
+        g.set_option("tangential", 1)
+    if rng.random() < 0.3:
+        g.set_option("strip", int(rng.integers(1, p.I + 1)))
+    g.set_state(W, f)
+    steps = int(rng.integers(1, 4))
+    g.step(steps); o.step(steps)
+    for _ in range(3):
+        name = ["chunk_m_m", "chunk_u", "R_m", "R_u", "strip_m", "strip_u"][int(rng.integers(0, 6))]
+        value = int(rng.integers(1, 40)) if name.startswith("chunk") else (int(rng.integers(1, 5)) if name.startswith("R") else int(rng.integers(1, p.I + 1)))
+        try:
+            g.set_option(name, value)
+        except UgksError:
+            pass                                                      # a geometry the library refuses (too many chunks, too many threads) is not applied
+        g.step(1); o.step(1)
+        steps += 1
+    r = _compare(g, o)
+    msg = "I %d J %d Nu %d Nv %d tangential %s: err_f %.3e err_W %.3e" % (p.I, p.J, p.Nu, p.Nv, tg, r["ef"], r["eW"])
+    assert r["ef"] <= steps * TOL_1 and r["eW"] <= steps * TOL_1, msg
+
+
 def test_rechunking_a_live_context_on_an_odd_grid():
     """The moment buffer is laid out per chunk and k_face_scalars reads entries k_cell_moments never writes (of the y- set of the chunk
     that holds the v = 0 row only three sums are stored): a new chunking of a context that has already stepped must start from a

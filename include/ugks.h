@@ -115,6 +115,33 @@ int ugks_kernel_times(ugks_ctx *, double ms[5], long counts[5]);
  * log (may be NULL) receives up to log_bytes of the compiler log, including ptxas' per-kernel register / shared-memory lines.
  * Returns UGKS_OK, UGKS_EINVAL (sizes) or UGKS_ECUDA (compile error: see log). */
 int ugks_jit_check(const ugks_mesh *, const ugks_vgrid *, const ugks_bcs *, char *log, size_t log_bytes);
+/* The L2 residual (RES row: north_star (iv), reading O11 of DESIGN.md; the W it measures is Eq. (4)'s) between two W
+ * fields, WITHOUT a context, a workspace or any allocation:
+ *     res[a] = sqrt(ncells * sum_c (W_new - W_old)[c][a]^2) / (sum_c |W_new[c][a]| + 1e-300),  a = 0..3.
+ * Meant for callers that cannot get device memory of their own: a convergence monitor or logging hook that only sees W^n and
+ * W^{n+1} inside a process whose whole device memory was handed to a pool up front (a raw cudaMalloc fails there although the
+ * pool has room, and the hook has no handle to the pool), or a time loop that cannot afford cudaMalloc / cudaFree because they
+ * synchronise the whole device.  The per-block partial sums, which ugks_residual keeps in the caller's workspace, go into a
+ * fixed array of UGKS_NOALLOC_SCRATCH_BYTES (512 KiB) inside the library image; every GPU that loads libugks.so holds that array
+ * until the process exits, whether or not this function is ever called.  The function calls no cudaMalloc, cudaFree or
+ * allocating library routine.
+ *   W_old, W_new  DEVICE pointers, [ncells][4] fp64 as everywhere in this header; read only, not retained.
+ *   ncells        1 .. UGKS_NOALLOC_MAX_CELLS (twice the cells of the largest BASELINE.json mesh); more -> UGKS_EINVAL, nothing launched.
+ *   res           DEVICE pointer to 4 doubles, written by the second of the two kernels this enqueues.
+ *   cuda_stream   cudaStream_t cast to void* (NULL = default stream) of the CURRENT device; the call is asynchronous and
+ *                 does not synchronise: read res after synchronising that stream.
+ *   err/err_bytes optional caller buffer for a message (NULL / 0: none); this function does not touch ugks_last_error().
+ * The first call on each device looks up that device's address of the array (cudaGetSymbolAddress, with the device current)
+ * and remembers it; make that first call before starting any stream capture.  All calls on a device share the one array and it
+ * keeps the previous call's partials: that is harmless for calls ordered on one stream or by events (every slot a call
+ * reads it has overwritten first, so nothing needs to start at zero), but two calls that overlap on the GPU -- different
+ * streams, no dependency -- race on it and both results are garbage.  Same block size and summation order as ugks_residual.
+ * Returns UGKS_OK, UGKS_EINVAL (NULL pointer, ncells out of range) or UGKS_ECUDA (no device, launch failure). */
+#define UGKS_NOALLOC_MAX_CELLS 1048576L
+#define UGKS_NOALLOC_SCRATCH_BYTES 524288
+int ugks_residual_noalloc(const double *W_old, const double *W_new, long ncells, double *res, void *cuda_stream,
+                          char *err, size_t err_bytes);
+
 const char *ugks_last_error(const ugks_ctx *);           /* library-owned string; ctx may be NULL */
 const char *ugks_version(void);
 void ugks_destroy(ugks_ctx *);

@@ -13,7 +13,9 @@ _dp = C.POINTER(C.c_double)
 
 EXPORTS = ["ugks_workspace_bytes", "ugks_init", "ugks_set_state", "ugks_step", "ugks_moments", "ugks_get_f",
            "ugks_residual", "ugks_sync", "ugks_dt", "ugks_mu_ref", "ugks_step_count", "ugks_launch_count",
-           "ugks_set_option", "ugks_kernel_times", "ugks_jit_check", "ugks_last_error", "ugks_version", "ugks_destroy"]
+           "ugks_set_option", "ugks_kernel_times", "ugks_jit_check", "ugks_last_error", "ugks_version", "ugks_destroy",
+           "ugks_residual_noalloc"]
+NOALLOC_MAX_CELLS = 1048576            # UGKS_NOALLOC_MAX_CELLS of include/ugks.h
 
 
 class UgksError(RuntimeError):
@@ -75,6 +77,7 @@ def lib():
         L.ugks_last_error.argtypes = [vp]; L.ugks_last_error.restype = C.c_char_p
         L.ugks_version.argtypes = []; L.ugks_version.restype = C.c_char_p
         L.ugks_destroy.argtypes = [vp]; L.ugks_destroy.restype = None
+        L.ugks_residual_noalloc.argtypes = [vp, vp, C.c_long, vp, vp, C.c_char_p, C.c_size_t]
         _lib = L
     return _lib
 
@@ -102,6 +105,29 @@ def jit_check(problem) -> str:
 def workspace_bytes(problem) -> int:
     keep, mesh, vg, gas, bcs = _structs(problem)
     return int(lib().ugks_workspace_bytes(C.byref(mesh), C.byref(vg)))
+
+
+def residual_noalloc(W_old, W_new, out=None, stream=None):
+    """ugks_residual_noalloc: the O11 residual between two W fields [..][4] (float64 torch CUDA tensors) without a context,
+    a workspace or any device allocation inside the library -- for code that cannot allocate (a monitoring hook in a
+    process whose device memory belongs to a pool, a loop that cannot take cudaMalloc's device-wide synchronisation).
+    The partial sums go to a fixed 512 KiB array inside libugks.so that all calls on a device share: keep calls ordered on
+    one stream.  ``out``: CUDA tensor of 4 doubles written asynchronously on ``stream`` (default: torch's current stream);
+    if None one is made HERE by torch (outside the library) and returned.  At most NOALLOC_MAX_CELLS cells."""
+    import torch
+    assert W_old.is_cuda and W_new.is_cuda and W_old.dtype == W_new.dtype == torch.float64
+    assert W_old.is_contiguous() and W_new.is_contiguous() and W_old.shape == W_new.shape and W_old.shape[-1] == 4
+    if out is None:
+        out = torch.empty(4, dtype=torch.float64, device=W_new.device)
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 4
+    st = stream if stream is not None else torch.cuda.current_stream(W_new.device)
+    buf = C.create_string_buffer(320)
+    with torch.cuda.device(W_new.device):
+        rc = lib().ugks_residual_noalloc(C.c_void_p(W_old.data_ptr()), C.c_void_p(W_new.data_ptr()), W_new.numel() // 4,
+                                         C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream), buf, len(buf))
+    if rc:
+        raise UgksError(rc, buf.value.decode(errors="replace"))
+    return out
 
 
 class Ugks:

@@ -34,16 +34,34 @@ KERNEL_ALG_BYTES = {"cell_moments": 8.0, "flux_update": 16.0}
 FP64_PEAK = 148 * 4 * 16 * 1.965e9  # plain FP64 pipe, thread-instructions/s (one warp DFMA per 2 cycles per sub-partition)
 
 
+COUNTS_FILE = "profiles/r3_counts.json"
+_KERNEL_SOURCES = ("ugks_jit_common.cuh", "ugks_jit_moments.cuh", "ugks_jit_update.cuh", "ugks_jit.cu", "ugks_api.cu")
+
+
+def kernel_source_sha():
+    """sha256 over the files that decide the code and the launch geometry of the two f-sized kernels."""
+    import hashlib
+    h = hashlib.sha256()
+    for fn in _KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_1810_08137_b200", "csrc", fn), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
 def _profile_counts(name):
-    """Per-kernel instruction counts and DRAM traffic of workload ``name`` from the committed ncu capture of this build
-    (profiles/r2_counts.json, written from `ncu --set full` by the command named in profiles/r2_kernels.md): FP64 thread
-    instructions (DFMA + DMUL + DADD, predicated on), all thread instructions, dram bytes -- per launch of one step.
-    None where no capture of that workload is committed (the figures are then reported as null, not guessed)."""
+    """Per-kernel instruction counts and DRAM traffic of workload ``name`` from the committed ncu capture (COUNTS_FILE, written
+    from the ncu command named in profiles/r3_kernels.md): FP64 thread instructions (DFMA + DMUL + DADD, predicated on), all
+    thread instructions, dram bytes -- per launch of one step.  The counts are static per build: the file records the sha256
+    of the kernel sources it was captured from, and (None, note) is returned when the sources here differ (a stale count would
+    otherwise be labelled "of this build") or when no capture of that workload is committed."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_counts.json")) as fh:
-            return json.load(fh).get(name)
+        with open(os.path.join(ROOT, COUNTS_FILE)) as fh:
+            d = json.load(fh)
     except Exception:
-        return None
+        return None, f"{COUNTS_FILE} missing"
+    if d.get("_meta", {}).get("kernel_source_sha256") != kernel_source_sha():
+        return None, f"{COUNTS_FILE} was captured from other kernel sources than this build's: instruction counts not reported"
+    return d.get(name), None if d.get(name) else f"no capture of {name} in {COUNTS_FILE}"
 
 
 def _cpu_model():
@@ -213,6 +231,18 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def _problem(name):
+    if name.startswith("M"):
+        mesh, nuv = name.split("-")
+        return workloads.paper_mesh(mesh, int(nuv))
+    return workloads.channel_config(name)
+
+
+def _summary_row(value, ms_step, hb, clocks):
+    return [float("%.4g" % value), round(ms_step, 4), round(hb["step_frac_of_16B_floor"], 4), round(hb["cell_moments"]["frac"], 4),
+            round(hb["flux_update"]["frac"], 4), clocks.get("sm_mhz")]
+
+
 def _workload_name(p):
     return f"{p.name}: channel {p.I}x{p.J} cells, {p.Nu}x{p.Nv} velocity grid, Kn={p.Kn}"
 
@@ -222,7 +252,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C4", choices=list(workloads.CONFIGS))
+    ap.add_argument("--config", default="C4", choices=list(workloads.CONFIGS) + ["M4-29", "M4-69", "M3-49"],
+                    help="BASELINE.json config, or one of the paper's own meshes x odd velocity grids (Table 1 / Table 3)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extra", action="store_true", help="skip the other configs / cpu baseline (N=1 default runs them)")
     ap.add_argument("--no-e2e", action="store_true")
@@ -247,12 +278,12 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    def measure(p, steps, warmup, e2e, kernels):
+    def measure(p, steps, warmup, e2e, kernels, tangential=False):
         fh = torch.empty((p.J, p.I, p.Nv, p.Nu), dtype=torch.float64, pin_memory=True)
         W, _, _ = workloads.initial_state(p, out_f=fh.numpy())          # f is drawn straight into pinned memory
         Wh = torch.from_numpy(W).pin_memory()
         del W
-        g = Ugks(p, device=dev)
+        g = Ugks(p, device=dev, tangential=tangential)
         g.set_state(Wh.to(dev), fh.to(dev))
         torch.cuda.empty_cache()
         g.step(warmup); g.sync()
@@ -292,7 +323,7 @@ def main():
         torch.cuda.empty_cache()
         return res
 
-    p = workloads.channel_config(args.config)
+    p = _problem(args.config)
     fp64_measured, fp64_3op = fp64_peak_measured()
 
     def hbm_fracs(q, ms_step, kernel_ms):
@@ -326,24 +357,27 @@ def main():
     kms = {k: v["ms_per_launch"] for k, v in r["kernels"].items()}      # per step (a kernel launched once per step and class)
     tot = sum(kms.values())
     dom = max(KERNEL_ALG_BYTES, key=lambda k: kms[k])
-    counts = _profile_counts(p.name)
+    counts, counts_note = _profile_counts(p.name)
     alu = alu_fracs(p, kms, counts)
     hbm = hbm_fracs(p, r["ms"] / steps, kms)
-    # The roof that binds this path is the plain FP64 pipe (and the issue slots that feed it), not HBM:
-    # roofline.{achieved, peak, frac} are the dominant kernel's FP64 thread-instructions per second against the measured DFMA
-    # rate; the HBM fractions north_star asks for are in roofline.hbm, for both f-sized kernels and for the step.
+    # roofline.{achieved, peak, frac}: the dominant kernel's ALGORITHMIC bytes (16 B per point-update for
+    # k_flux_update -- f^n read once, f^{n+1} written once) over its CUDA-event time against the measured HBM peak: the number
+    # north_star's 60 % bar is read against.  What actually binds the kernel is the plain FP64 pipe: its
+    # utilisation (EXECUTED FP64 thread-instructions per second against the measured DFMA rate) is in roofline.pipe_util.
+    roof = {"bound": "hbm", "kernel": dom, "achieved": hbm[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
+            "frac": hbm[dom]["frac"], "traffic": (counts or {}).get(dom, {}).get("dram_bytes"), "peak_source": peak_src,
+            "alg_bytes_per_launch": KERNEL_ALG_BYTES[dom] * p.points,
+            "step_frac_of_16B_floor": hbm["step_frac_of_16B_floor"], "step_frac_of_declared_24B": hbm["step_frac_of_declared_24B"],
+            "binding_roof": "fp64 pipe (see pipe_util): at the executed FP64 instructions per update the pipe alone caps the step below the HBM floor"}
     if alu and dom in alu:
-        roof = {"bound": "alu", "kernel": dom, "achieved": alu[dom]["fp64_inst_per_s"] / 1e12, "peak": fp64_measured / 1e12,
-                "unit": "T FP64 thread-inst/s", "frac": alu[dom]["frac_of_fp64_peak"], "traffic": alu[dom]["dram_bytes"],
-                "peak_source": "measured here: bench_fp64_peak.cu, 8 independent DFMA chains per thread (nominal 148 SMs x 4 x 16 lanes x 1.965 GHz = %.3g)" % FP64_PEAK,
-                "peak_3operand": fp64_3op / 1e12, "frac_of_3operand": alu[dom]["fp64_inst_per_s"] / fp64_3op,
-                "peak_3operand_source": "measured here: 32 accumulators, x[i] += x[i+5] * x[i+11] (three distinct register operands per DFMA): the rate "
-                                        "register-operand fetch allows; context for frac, not its denominator",
-                "counts_source": "profiles/r2_counts.json (ncu --set full of this build, static per build; times are live)"}
+        roof["pipe_util"] = {"kernel": dom, "achieved": alu[dom]["fp64_inst_per_s"] / 1e12, "peak": fp64_measured / 1e12,
+                             "unit": "T executed FP64 thread-inst/s", "frac": alu[dom]["frac_of_fp64_peak"],
+                             "peak_source": "measured here: bench_fp64_peak.cu, 8 independent DFMA chains per thread (nominal 148 SMs x 4 x 16 lanes x 1.965 GHz = %.3g)" % FP64_PEAK,
+                             "peak_3operand": fp64_3op / 1e12, "frac_of_3operand": alu[dom]["fp64_inst_per_s"] / fp64_3op,
+                             "counts_source": COUNTS_FILE + " (ncu counters of the kernel sources with the recorded sha256; static per build, times are live)"}
     else:
-        roof = {"bound": "hbm", "kernel": dom, "achieved": hbm[dom]["achieved_gbs"], "peak": peak, "unit": "GB/s",
-                "frac": hbm[dom]["frac"], "traffic": None, "peak_source": peak_src,
-                "note": "no committed instruction counts for this workload: HBM fraction of the dominant kernel reported"}
+        roof["pipe_util"] = None
+        roof["pipe_util_note"] = counts_note
     roof.update({"hbm": dict(hbm, peak_gbs=peak, peak_source=peak_src), "alu": alu,
                  "kernel_share_of_step": kms[dom] / tot, "kernel_ms": {k: round(v, 5) for k, v in kms.items()}})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
@@ -359,13 +393,17 @@ def main():
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "cpu": _cpu_model(),
                                 "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "sample": sample1}}
         others = {}
+        summary = {p.name: _summary_row(value, r["ms"] / steps, hbm, r["clocks"])}
 
-        def other(q, st, label):
-            rr = measure(q, st, 3, e2e=False, kernels=True)
+        def other(q, st, label, tangential=False):
+            rr = measure(q, st, 3, e2e=False, kernels=True, tangential=tangential)
             km = {k: v["ms_per_launch"] for k, v in rr["kernels"].items()}
-            others[q.name] = {"value": q.points * st / (rr["ms"] * 1e-3), "ms_per_step": rr["ms"] / st, "steps": st, "workload": label,
-                              "clocks": rr["clocks"], "kernel_ms": {k: round(v, 5) for k, v in km.items()},
-                              "hbm": hbm_fracs(q, rr["ms"] / st, km), "alu": alu_fracs(q, km, _profile_counts(q.name))}
+            key = q.name + ("-tangential" if tangential else "")
+            hb = hbm_fracs(q, rr["ms"] / st, km)
+            others[key] = {"value": q.points * st / (rr["ms"] * 1e-3), "ms_per_step": rr["ms"] / st, "steps": st, "workload": label,
+                           "clocks": rr["clocks"], "kernel_ms": {k: round(v, 5) for k, v in km.items()},
+                           "hbm": hb, "alu": None if tangential else alu_fracs(q, km, _profile_counts(q.name)[0])}
+            summary[key] = _summary_row(others[key]["value"], rr["ms"] / st, hb, rr["clocks"])
         for name in workloads.CONFIGS:
             if name == args.config or name == "C1":
                 continue
@@ -377,7 +415,12 @@ def main():
         for mname, nuv, st in (("M4", 29, 100), ("M4", 69, 40), ("M3", 49, 40)):         # the paper's own shapes (Table 1 / Table 3)
             q = workloads.paper_mesh(mname, nuv)
             other(q, st, f"paper mesh {mname} {q.I}x{q.J}, {nuv}x{nuv} velocity grid, Kn=0.1")
+        # option "tangential" on the headline workload: its own clocks and kernel fractions
+        other(p, max(5, steps // 2), _workload_name(p) + ", option tangential (O3t/O8t)", tangential=True)
         line["other_workloads"] = others
+        # one compact row per workload at the END of the line, so that a truncated tail still carries every workload:
+        # [updates/s, ms per step, step / 16-B floor, cell_moments HBM frac (8 B/pt), flux_update HBM frac (16 B/pt), median SM MHz]
+        line["workload_summary"] = summary
     if rank == 0:
         print(json.dumps(line), flush=True)
     if dist is not None:

@@ -42,7 +42,8 @@ enum { UGKS_BC_PERIODIC = 0, UGKS_BC_FIXED = 1, UGKS_BC_WALL = 2 };
 /* Uniform Cartesian mesh of I x J control volumes.  I, J >= 2. */
 typedef struct { int I, J; double x0, x1, y0, y1; } ugks_mesh;
 /* Discrete velocity grid K x M of the paper = Nu x Nv here.  HOST arrays, copied at init.
- * 1 <= Nu <= 512 (a CTA has one thread per column of the velocity grid and keeps 128 registers per thread up to 512 threads), 1 <= Nv <= 4096.
+ * 1 <= Nu <= 512 (a CTA has one thread per column of the velocity grid and keeps 128 registers per thread up to 512 threads), 1 <= Nv <= 2048 (the nodes, weights and the row-chunk table
+ * of the run-time compiled kernels live in the 64 KB constant bank).  All nodes and weights must be finite;
  * Weights must have positive sums. */
 typedef struct { int Nu, Nv; const double *u, *wu, *v, *wv; } ugks_vgrid;
 /* Gas: viscosity exponent omega (mu = mu_ref T^omega), mu_ref (<= 0: derive from Kn, AMB-7),

@@ -1,6 +1,9 @@
 """Build libugks.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_1810_08137_b200.build [--force] [--verbose]
+    python -m paper_1810_08137_b200.build [--force] [--verbose] [--developer]
+
+--developer compiles with -DUGKS_DEVELOPER: the library then honours the UGKS_* environment overrides used for experiments and
+SASS dumps (see csrc/ugks_jit.cu).  The default build reads no environment variable.
 """
 from __future__ import annotations
 
@@ -24,7 +27,7 @@ def _deps():
     return sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "ugks.h")]
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, developer: bool = False) -> str:
     stale = force or not os.path.exists(SO) or any(os.path.getmtime(s) > os.path.getmtime(SO) for s in _deps())
     if not stale:
         return SO
@@ -32,6 +35,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
     if verbose:
         flags += ["-Xptxas", "-v"]
+    if developer:
+        flags += ["-DUGKS_DEVELOPER"]
     tmp = SO + f".tmp{os.getpid()}"
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
@@ -56,4 +61,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv or "--developer" in sys.argv, verbose="--verbose" in sys.argv, developer="--developer" in sys.argv))

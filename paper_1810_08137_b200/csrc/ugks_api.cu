@@ -28,7 +28,7 @@ struct ugks_ctx {
     cudaEvent_t *ev; int nev, nev_used;
     double kms[5]; long kcnt[5];
     // CUDA graph of two consecutive steps (launch-bound meshes): captured on an internal stream, replayed between two events
-    int graph_mode;           // option "graph": -1 auto (on below 4e6 points per step), 0 off, 1 on
+    int graph_mode;           // option "graph": -1 auto (on below 3e7 points per step), 0 off, 1 on
     long graph_launches;      // kernels inside a graph
     cudaStream_t gst; cudaGraphExec_t gexec[2]; cudaEvent_t gin, gout;       // gexec[p]: two steps starting from state parity p
     char err[256];
@@ -67,6 +67,7 @@ static size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 // is uniform over a CTA), each run into equal chunks of at most `cm_target` rows; rows with v = 0 and, if the node order makes
 // too many runs, everything, go to "mixed" chunks that select the side per point.  Order: [v < 0][v > 0][mixed].
 constexpr int MAXCHUNK = 4096;
+constexpr int MAXNV = 2048;                                          // c_v, c_wv and the chunk table of the generated kernels share the 64 KB constant bank
 constexpr int MAXNU = 512;                                           // one thread per column: a CTA of <= 512 threads keeps 128 registers per thread
 
 static void make_chunks(const double *v, int Nv, int Nu, int cm_target, KGeom *G)
@@ -135,7 +136,6 @@ static void set_u_ranges(UgksParams &T, const double *uhost)
         k1 = k0; while (k1 < T.Nu && uhost[k1] <= 0.0) ++k1;         // first u > 0
         T.kxp_begin = k0; T.kxm_end = k1;
     }
-    T.s3_nsx = T.s3_nsy = 0;                                         // (the stage-3 split is a compile-time constant of the kernel)
 }
 // default launch geometry of kernel `kind` for the sizes, node signs and options (tangential) in T: the largest chunk of at
 // most the target rows whose CTA fits the 227 KB of shared memory
@@ -197,9 +197,21 @@ struct Layout {
         chunks, bcprim, Wf, total;
     int Npad, resblocks, NuP, NvP, frs, crs, nchunk_alloc;
 };
+// nodes and weights become literals of the generated kernel source and decide the chunking: NaN / Inf are refused up front
+static bool all_finite(const double *a, int n)
+{
+    for (int i = 0; i < n; ++i) if (!isfinite(a[i])) return false;
+    return true;
+}
+static bool vgrid_finite(const ugks_vgrid *vg)
+{
+    return all_finite(vg->u, vg->Nu) && all_finite(vg->wu, vg->Nu) && all_finite(vg->v, vg->Nv) && all_finite(vg->wv, vg->Nv);
+}
+// __constant__ bytes of a generated kernel: c_u, c_wu, c_v, c_wv and the chunk table; the bank holds 64 KB
+static size_t jit_const_bytes(const UgksParams &T, const KGeom &G) { return 16 * ((size_t)T.Nu + T.Nv) + 16 * (size_t)G.nchunk(); }
 static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
 {
-    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > MAXNU || vg->Nv < 1 || vg->Nv > MAXCHUNK) return 1;
+    if (!m || !vg || m->I < 2 || m->J < 2 || vg->Nu < 1 || vg->Nu > MAXNU || vg->Nv < 1 || vg->Nv > MAXNV) return 1;
     const size_t cells = (size_t)m->I * m->J, N = (size_t)vg->Nu * vg->Nv;
     const size_t Npad = (N + 15) & ~(size_t)15;
     const size_t nfx = (size_t)(m->I + 1) * m->J, nfy = (size_t)m->I * (m->J + 1);
@@ -217,6 +229,9 @@ static int make_layout(const ugks_mesh *m, const ugks_vgrid *vg, Layout *L)
         KGeom G;
         choose_geometry(JIT_MOMENTS, T, vg->v, &G);
         if ((size_t)G.nchunk() > nchunk) nchunk = (size_t)G.nchunk();
+        KGeom Gu;
+        choose_geometry(JIT_UPDATE, T, vg->v, &Gu);
+        if (jit_const_bytes(T, G) > 65536 || jit_const_bytes(T, Gu) > 65536) return 1;   // ugks_init could not compile its kernels
     }
     if (nchunk < 1 || nchunk > MAXCHUNK) return 1;
     L->nchunk_alloc = (int)nchunk;
@@ -249,6 +264,7 @@ static const char *check_geometry(int kind, const UgksParams &T, const KGeom &G)
     if (G.npt < 1 || G.npt > 16 || G.R < 1 || T.Nu * G.R > MAXNU || G.R * G.npt < G.cmax) return "R / points per thread out of range";
     if (G.strip < 0 || G.strip > T.I) return "strip out of range (0 = automatic, else 1..I)";
     if (jit_smem(kind, T, G) > 227 * 1024) return "chunk does not fit in shared memory";
+    if (jit_const_bytes(T, G) > 65536) return "velocity nodes, weights and chunk table exceed the 64 KB constant bank";
     return nullptr;
 }
 
@@ -266,22 +282,28 @@ static int apply_geometry(ugks_ctx *c, int kind, const KGeom &G)
     char msg[240];
     KGeom Gs = G;
     const bool auto_strip = Gs.strip == 0;
-    if (auto_strip) Gs.strip = default_strip(T.I);
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    // automatic strip (few waves on small meshes, choose_strip): first from the occupancy the kernel is compiled FOR (launch bounds:
+    // known on the host), so that one compile suffices; the compiled kernel's own occupancy then has the last word -- only if
+    // it asks for another strip is the kernel compiled a second time
+    if (auto_strip) Gs.strip = choose_strip(T.I, T.J, G.nchunk(), jit_ctas_estimate(kind, T, G), sms, default_strip(T.I));
     if (jit_get(kind, T, Gs, c->uhost, c->wuhost, c->vhost, c->wvhost, &jk, msg, sizeof msg)) return fail(c, UGKS_ECUDA, "%s", msg);
-    if (auto_strip) {                                                // few waves: pick the strip from this kernel's occupancy, re-compile
-        int sms = 148;
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
-        const int s = choose_strip(T.I, T.J, G.nchunk(), jit_ctas_per_sm(jk), sms, Gs.strip);
+    if (auto_strip) {
+        const int s = choose_strip(T.I, T.J, G.nchunk(), jit_ctas_per_sm(jk), sms, default_strip(T.I));
         if (s != Gs.strip) {
+            jit_release(jk);
             Gs.strip = s;
             if (jit_get(kind, T, Gs, c->uhost, c->wuhost, c->vhost, c->wvhost, &jk, msg, sizeof msg)) return fail(c, UGKS_ECUDA, "%s", msg);
         }
     }
     const KGeom &G2 = Gs;
+#ifdef UGKS_DEVELOPER
     if (getenv("UGKS_DEBUG"))
         fprintf(stderr, "ugks: %s geometry: %d chunks (cmax %d), R %d, %d points/thread, strip %d, %d CTAs/SM, %d threads, %zu B smem\n",
                 kind == JIT_MOMENTS ? "k_cell_moments" : "k_flux_update", G.nchunk(), G.cmax, G.R, G.npt, G2.strip, jit_ctas_per_sm(jk), jk->threads,
                 jit_smem(kind, T, G));
+#endif
     if (kind == JIT_MOMENTS) {
         // the moment buffer is laid out per chunk, and k_face_scalars reads entries that k_cell_moments never writes (of the y- set
         // of the chunk that holds a v = 0 row only M00, M01, M02 are stored; the T sums without option "tangential"): they must be
@@ -290,8 +312,8 @@ static int apply_geometry(ugks_ctx *c, int kind, const KGeom &G)
         CK(cudaMemcpy(c->chunks_dev, G.chunks.data(), sizeof(int4) * G.nchunk(), cudaMemcpyHostToDevice), "apply_geometry");
         T.nchunk = G.nchunk(); T.nneg = G.nneg; T.npos = G.npos; T.nmix = G.nmix; T.cmax = G.cmax; T.R = G.R; T.npt = G.npt; T.strip = G2.strip;
         c->P = T;
-        *c->gm = G2; c->km = jk;
-    } else { *c->gu = G2; c->ku = jk; }
+        *c->gm = G2; jit_release(c->km); c->km = jk;
+    } else { *c->gu = G2; jit_release(c->ku); c->ku = jk; }
     return UGKS_OK;
 }
 
@@ -305,6 +327,7 @@ int ugks_jit_check(const ugks_mesh *m, const ugks_vgrid *vg, const ugks_bcs *bcs
     if (log && log_bytes) log[0] = 0;
     Layout L;
     if (!bcs || make_layout(m, vg, &L) || !vg->u || !vg->wu || !vg->wv) return fail(nullptr, UGKS_EINVAL, "%s", "invalid mesh or velocity grid");
+    if (!vgrid_finite(vg)) return fail(nullptr, UGKS_EINVAL, "%s", "velocity nodes and weights must be finite");
     UgksParams T;
     memset(&T, 0, sizeof T);
     T.I = m->I; T.J = m->J; T.Nu = vg->Nu; T.Nv = vg->Nv; T.N = vg->Nu * vg->Nv; T.Npad = L.Npad;
@@ -312,7 +335,9 @@ int ugks_jit_check(const ugks_mesh *m, const ugks_vgrid *vg, const ugks_bcs *bcs
     const ugks_bc *b[4] = { &bcs->xmin, &bcs->xmax, &bcs->ymin, &bcs->ymax };
     for (int s = 0; s < 4; ++s) T.bc[s] = b[s]->type;
     set_u_ranges(T, vg->u);
-    if (const char *e = getenv("UGKS_JIT_CHECK_TANGENTIAL")) T.tangential = atoi(e) != 0;      // developer aid: check the TG variants
+#ifdef UGKS_DEVELOPER
+    if (const char *e = getenv("UGKS_JIT_CHECK_TANGENTIAL")) T.tangential = atoi(e) != 0;      // check the TG variants
+#endif
     std::string all;
     for (int kind = 0; kind < 2; ++kind) {
         KGeom G;
@@ -343,9 +368,10 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     *out = nullptr;
     if (!m || !vg || !gas || !bcs || !workspace_dev) return fail(c, UGKS_EINVAL, "%s", "NULL argument");
     Layout L;
-    if (make_layout(m, vg, &L)) return fail(c, UGKS_EINVAL, "%s", "invalid mesh or velocity grid size (I,J >= 2; 1 <= Nu <= 512)");
+    if (make_layout(m, vg, &L)) return fail(c, UGKS_EINVAL, "%s", "invalid mesh or velocity grid size (I,J >= 2; 1 <= Nu <= 512; 1 <= Nv <= 2048)");
     if (!(m->x1 > m->x0) || !(m->y1 > m->y0)) return fail(c, UGKS_EINVAL, "%s", "empty domain");
     if (!vg->u || !vg->wu || !vg->v || !vg->wv) return fail(c, UGKS_EINVAL, "%s", "NULL velocity arrays");
+    if (!vgrid_finite(vg)) return fail(c, UGKS_EINVAL, "%s", "velocity nodes and weights must be finite");
     if (gas->Pr != 1.0) return fail(c, UGKS_EINVAL, "%s", "Pr must be 1 (BGK)");
     if (gas->K_int != 0) return fail(c, UGKS_EINVAL, "%s", "K_int must be 0");
     if (!(cfl > 0.0)) return fail(c, UGKS_EINVAL, "%s", "cfl must be positive");
@@ -440,7 +466,7 @@ int ugks_init(ugks_ctx **out, const ugks_mesh *m, const ugks_vgrid *vg, const ug
     if (e != cudaSuccess) { int rc = cuda_fail(nullptr, e, "ugks_init"); delete c->gm; delete c->gu; free(c->vhost); free(c); return rc; }
     for (int kind = 0; kind < 2; ++kind) {
         const int rc = apply_geometry(c, kind, G0[kind]);
-        if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); delete c->gm; delete c->gu; free(c->vhost); free(c); return rc; }
+        if (rc) { snprintf(g_err, sizeof g_err, "%s", c->err); jit_release(c->km); jit_release(c->ku); delete c->gm; delete c->gu; free(c->vhost); free(c); return rc; }
     }
     *out = c;
     return UGKS_OK;
@@ -455,6 +481,8 @@ void ugks_destroy(ugks_ctx *c)
     for (int i = 0; i < c->nev; ++i) cudaEventDestroy(c->ev[i]);
     free(c->ev);
     free(c->vhost);
+    jit_release(c->km);
+    jit_release(c->ku);
     delete c->gm;
     delete c->gu;
     free(c);

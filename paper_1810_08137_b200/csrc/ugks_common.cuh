@@ -37,7 +37,8 @@ enum { LR_C10 = 0, LR_C20 = 1, LR_C30 = 2, LR_C11 = 3, LR_C12 = 4 };
 //   [0, CR_NCOEF)                          see CR_*
 //   [CR_NCOEF, +NuP)                       gn_u[k] = GN exp(-lam_n (u_k - U_n)^2)    (relaxation prefactors folded in)
 //   [CR_NCOEF + NuP, +NuP)                 gp_u[k] = GP exp(-lam_p (u_k - U_p)^2)
-//   [CR_NCOEF + 2 NuP, +2 Nv)              pairs (gn_v[m], gp_v[m]) = (exp(-lam_n (v_m - V_n)^2), exp(-lam_p (v_m - V_p)^2))
+//   [CR_NCOEF + 2 NuP, +NvP)               gn_v[m] = exp(-lam_n (v_m - V_n)^2)
+//   [CR_NCOEF + 2 NuP + NvP, +NvP)         gp_v[m] = exp(-lam_p (v_m - V_p)^2)
 constexpr int CR_NCOEF = 12;
 enum { CR_KF = 0, CR_KD = 1, CR_GN = 2, CR_GP = 3, CR_UN = 4, CR_VN = 5, CR_LN = 6, CR_UP = 7, CR_VP = 8, CR_LP = 9 };
 
@@ -71,7 +72,6 @@ struct UgksParams {
     int R;                           // velocity rows processed in parallel by one CTA (threads = Nu*R rounded up to 32)
     int npt;                         // velocity points per thread = ceil(cmax / R), 1..16 (compile-time constant of the JIT kernels)
     int kxm_end, kxp_begin;          // columns with u_k <= 0 are [0, kxm_end), with u_k >= 0 [kxp_begin, Nu) (sorted nodes; else 0..Nu)
-    int s3_nsx, s3_nsy;              // unused (the stage-3 split of k_cell_moments is a compile-time constant)
 };
 
 static __host__ __device__ inline int nfaces_x(const UgksParams &P) { return (P.I + 1) * P.J; }

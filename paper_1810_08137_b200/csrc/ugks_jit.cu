@@ -24,12 +24,35 @@ namespace {
 
 std::mutex g_mu;
 std::map<std::string, JitKernel *> g_cache;
+unsigned long g_tick = 0;
+
+// unload unused kernels, least recently used first, until at most JIT_CACHE_MAX entries remain (g_mu held)
+void evict_unused()
+{
+    while ((int)g_cache.size() > JIT_CACHE_MAX) {
+        auto victim = g_cache.end();
+        for (auto it = g_cache.begin(); it != g_cache.end(); ++it)
+            if (it->second->users == 0 && (victim == g_cache.end() || it->second->last_used < victim->second->last_used)) victim = it;
+        if (victim == g_cache.end()) return;                        // every cached kernel is in use
+        if (victim->second->lib) cudaLibraryUnload(victim->second->lib);
+        delete victim->second;
+        g_cache.erase(victim);
+    }
+}
 
 int pad2i(int x) { return (x + 1) & ~1; }
 int cdivi(int a, int b) { return (a + b - 1) / b; }
 
 // host mirrors of MomL<MIXED>::BYTES and StageL<NY>::BYTES (the device code static_asserts that they agree)
-int nsxm() { const char *e = getenv("UGKS_NSXM"); const int n = e ? atoi(e) : 3; return n < 2 ? 2 : (n > 4 ? 4 : n); }   // x-ring slots of k_cell_moments
+// Environment overrides exist only in a developer build (python -m paper_1810_08137_b200.build --developer => -DUGKS_DEVELOPER):
+// UGKS_NSXM, UGKS_SLICE, UGKS_JIT_DEFS (extra #define lines), UGKS_JIT_MAXREG, UGKS_JIT_DUMP (keep the cubins for cuobjdump),
+// UGKS_DEBUG, UGKS_JIT_CHECK_TANGENTIAL.  The shipped library reads no environment variable.
+#ifdef UGKS_DEVELOPER
+const char *dev_env(const char *name) { return getenv(name); }
+#else
+const char *dev_env(const char *) { return nullptr; }
+#endif
+int nsxm() { const char *e = dev_env("UGKS_NSXM"); const int n = e ? atoi(e) : 3; return n < 2 ? 2 : (n > 4 ? 4 : n); }   // x-ring slots of k_cell_moments
 int smem_mom_q(const UgksParams &P, const KGeom &G, bool mixed, int QB);
 int smem_upd_q(const UgksParams &P, const KGeom &G, int ny, int QB);
 bool upd_slice(const UgksParams &P, const KGeom &G);
@@ -60,10 +83,10 @@ int smem_mom_q(const UgksParams &P, const KGeom &G, bool mixed, int QB)
 }
 int smem_upd(const UgksParams &P, const KGeom &G, int ny) { return smem_upd_q(P, G, ny, qb_of(JIT_UPDATE, P, G)); }
 // k_flux_update stages, of the v-tables of a face / cell record, only the rows of its chunk when that saves at least 64 doubles
-// per table (SLICE in ugks_jit_update.cuh; developer override UGKS_SLICE=0/1)
+// per table (SLICE in ugks_jit_update.cuh)
 bool upd_slice(const UgksParams &P, const KGeom &G)
 {
-    if (const char *e = getenv("UGKS_SLICE")) return atoi(e) != 0;
+    if (const char *e = dev_env("UGKS_SLICE")) return atoi(e) != 0;
     return P.NvP - pad2i(G.cmax + 1) >= 64;
 }
 int smem_upd_q(const UgksParams &P, const KGeom &G, int ny, int QB)
@@ -108,12 +131,33 @@ bool read_file(const std::string &path, std::string *out)
     return true;
 }
 
+// exact hexadecimal floating literal of a finite double, built from its bits: unlike printf("%a") it does not depend on the
+// host application's LC_NUMERIC (a comma radix would break the generated source)
+void hex_literal(double x, char out[40])
+{
+    unsigned long long b;
+    memcpy(&b, &x, 8);
+    const int e = (int)((b >> 52) & 0x7ff);
+    const unsigned long long m = b & 0xfffffffffffffULL;
+    const char *sg = (b >> 63) ? "-" : "";
+    if (e == 0) snprintf(out, 40, "%s0x0.%013llxp-1022", sg, m);          // zero and subnormals
+    else snprintf(out, 40, "%s0x1.%013llxp%+d", sg, m, e - 1023);
+}
 void add_doubles(std::string &s, const char *name, const double *a, int n)
 {
-    char buf[64];
+    char buf[40];
     s += "__constant__ double "; s += name; s += "[] = {";
-    for (int i = 0; i < n; ++i) { snprintf(buf, sizeof buf, "%s%a", i ? ", " : "", a[i]); s += buf; }
+    for (int i = 0; i < n; ++i) { hex_literal(a[i], buf); if (i) s += ", "; s += buf; }
     s += "};\n";
+}
+// the first line of a compiler log that reports an error (the log starts with ptxas info lines), else its head
+std::string first_error_line(const std::string &log)
+{
+    size_t at = log.find("error");
+    if (at == std::string::npos) return log.substr(0, 200);
+    size_t b = log.rfind('\n', at), e = log.find('\n', at);
+    b = b == std::string::npos ? 0 : b + 1;
+    return log.substr(b, (e == std::string::npos ? log.size() : e) - b).substr(0, 200);
 }
 
 }  // namespace
@@ -150,7 +194,7 @@ std::string jit_prelude(int kind, const UgksParams &P, const KGeom &G, const dou
     s += "__constant__ int4 c_chunks[] = {";
     for (int i = 0; i < G.nchunk(); ++i) { snprintf(b, sizeof b, "%s{%d, %d, %d, %d}", i ? ", " : "", G.chunks[i].x, G.chunks[i].y, G.chunks[i].z, G.chunks[i].w); s += b; }
     s += "};\n";
-    if (const char *extra = getenv("UGKS_JIT_DEFS")) { s += extra; s += "\n"; }      // developer aid: extra #define lines for experiments
+    if (const char *extra = dev_env("UGKS_JIT_DEFS")) { s += extra; s += "\n"; }     // developer build only
     add_doubles(s, "c_u", u, P.Nu); add_doubles(s, "c_wu", wu, P.Nu); add_doubles(s, "c_v", v, P.Nv); add_doubles(s, "c_wv", wv, P.Nv);
     return s;
 }
@@ -169,7 +213,7 @@ int jit_compile(int kind, const std::string &prelude, std::vector<char> *cubin, 
     std::vector<const char *> opts = { "--gpu-architecture=sm_100a", "-lineinfo", "--std=c++17", "-default-device", inc.c_str() };
     if (verbose) opts.push_back("--ptxas-options=-v");
     std::string maxreg;
-    if (const char *e = getenv("UGKS_JIT_MAXREG")) { maxreg = std::string("--maxrregcount=") + e; opts.push_back(maxreg.c_str()); }   // developer aid
+    if (const char *e = dev_env("UGKS_JIT_MAXREG")) { maxreg = std::string("--maxrregcount=") + e; opts.push_back(maxreg.c_str()); }   // developer build only
     const nvrtcResult rc = nvrtcCompileProgram(prog, (int)opts.size(), opts.data());
     size_t n = 0;
     nvrtcGetProgramLogSize(prog, &n);
@@ -180,7 +224,7 @@ int jit_compile(int kind, const std::string &prelude, std::vector<char> *cubin, 
     cubin->resize(n);
     nvrtcGetCUBIN(prog, cubin->data());
     nvrtcDestroyProgram(&prog);
-    if (const char *dump = getenv("UGKS_JIT_DUMP")) {               // keep the image for cuobjdump -sass: <dump>.moments.cubin / <dump>.update.cubin
+    if (const char *dump = dev_env("UGKS_JIT_DUMP")) {               // keep the image for cuobjdump -sass: <dump>.moments.cubin / <dump>.update.cubin
         const std::string path = std::string(dump) + (kind == JIT_MOMENTS ? ".moments.cubin" : ".update.cubin");
         if (FILE *f = fopen(path.c_str(), "wb")) { fwrite(cubin->data(), 1, cubin->size(), f); fclose(f); }
     }
@@ -191,7 +235,8 @@ int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, cons
             JitKernel **out, char *err, size_t errlen)
 {
     const std::string pre = jit_prelude(kind, P, G, u, wu, v, wv);
-    const std::string key = (kind == JIT_MOMENTS ? "M:" : "U:") + pre;
+    std::string key = (kind == JIT_MOMENTS ? "M:" : "U:") + pre;
+    if (const char *e = dev_env("UGKS_JIT_MAXREG")) { key += "//maxreg="; key += e; }   // changes the cubin, so it is part of the key
     std::lock_guard<std::mutex> lock(g_mu);
     JitKernel *m = nullptr;
     auto it = g_cache.find(key);
@@ -199,7 +244,7 @@ int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, cons
     else {
         std::vector<char> cubin;
         std::string log;
-        if (jit_compile(kind, pre, &cubin, &log, false)) { snprintf(err, errlen, "JIT compile failed: %.200s", log.c_str()); return 1; }
+        if (jit_compile(kind, pre, &cubin, &log, false)) { snprintf(err, errlen, "JIT compile failed: %s", first_error_line(log).c_str()); return 1; }
         m = new JitKernel();
         m->image.swap(cubin);
         cudaError_t e = cudaLibraryLoadData(&m->lib, m->image.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
@@ -211,12 +256,30 @@ int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, cons
         else m->smem = smem_upd(P, G, G.nmix > 0 ? 4 : (P.tangential ? 6 : 3));
         g_cache[key] = m;
     }
+    m->users += 1;
+    m->last_used = ++g_tick;
+    evict_unused();
     // shared-memory opt-in: a function attribute of the CURRENT device, set for every context (cheap, idempotent)
     cudaError_t e = cudaFuncSetAttribute((const void *)m->k, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smem);
     if (e == cudaSuccess && m->kx) e = cudaFuncSetAttribute((const void *)m->kx, cudaFuncAttributeMaxDynamicSharedMemorySize, m->smemx);
-    if (e != cudaSuccess) { snprintf(err, errlen, "shared-memory opt-in failed: %s", cudaGetErrorString(e)); return 1; }
+    if (e != cudaSuccess) { m->users -= 1; snprintf(err, errlen, "shared-memory opt-in failed: %s", cudaGetErrorString(e)); return 1; }
     *out = m;
     return 0;
+}
+
+void jit_release(JitKernel *m)
+{
+    if (!m) return;
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (m->users > 0) m->users -= 1;
+    evict_unused();
+}
+
+int jit_ctas_estimate(int kind, const UgksParams &P, const KGeom &G)
+{
+    const int threads = threads_of(kind, P, G);
+    if (kind == JIT_MOMENTS) return min_blocks(threads, smem_mom(P, G, G.nmix > 0), 128);
+    return min_blocks(threads, G.nmix > 0 ? smem_upd(P, G, 4) : smem_upd(P, G, P.tangential ? 6 : 3), 128);
 }
 
 // CTAs of this kernel that one SM holds (registers, shared memory, threads) on the current device

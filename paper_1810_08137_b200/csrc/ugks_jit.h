@@ -25,6 +25,8 @@ struct JitKernel {
     cudaLibrary_t lib = nullptr;
     cudaKernel_t k = nullptr, kx = nullptr;      // the kernel; for JIT_MOMENTS also the variant for mixed-sign chunks
     int threads = 0, smem = 0, smemx = 0;
+    int users = 0;                   // contexts holding this kernel (jit_get takes a reference, jit_release drops it)
+    unsigned long last_used = 0;     // for the eviction order of unused kernels
 };
 
 // dynamic shared memory of a kernel of this geometry (the larger of its variants)
@@ -34,6 +36,13 @@ int jit_compile(int kind, const std::string &prelude, std::vector<char> *cubin, 
 // kernel for this geometry (compiled once per process and prelude); sets the shared-memory opt-in on the current device
 int jit_get(int kind, const UgksParams &P, const KGeom &G, const double *u, const double *wu, const double *v, const double *wv,
             JitKernel **out, char *err, size_t errlen);
+// drop the reference jit_get took.  Kernels nobody holds stay cached for the next context of that geometry, up to JIT_CACHE_MAX
+// of them; beyond that the least recently used ones are unloaded (cudaLibraryUnload) and freed.
+void jit_release(JitKernel *m);
+constexpr int JIT_CACHE_MAX = 32;
 int jit_ctas_per_sm(const JitKernel *m);
+// CTAs per SM the kernel of this geometry is compiled for (__launch_bounds__): min(shared memory, 128 registers per thread);
+// known without compiling, a lower bound of jit_ctas_per_sm
+int jit_ctas_estimate(int kind, const UgksParams &P, const KGeom &G);
 int jit_launch_cell_moments(const JitKernel *m, const UgksParams &P, const KGeom &G, int cur, cudaStream_t st);
 int jit_launch_flux_update(const JitKernel *m, const UgksParams &P, const KGeom &G, int cur, cudaStream_t st);

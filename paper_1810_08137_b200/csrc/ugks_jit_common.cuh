@@ -4,8 +4,8 @@
 // compile-time constants (the G_* macros of a generated prelude: mesh and velocity-grid sizes, boundary types, the
 // velocity-row chunking, R / NPT, strip length, record strides; the velocity nodes, weights and the chunk table come as
 // __constant__ arrays).  Every stride, trip count and job table below is therefore an immediate: the per-cell control code of
-// the marching CTAs (about half of all executed instructions with run-time geometry, profiles/r1c_kernels.md) folds away.
-// The same file compiles under nvcc with a sample prelude (ugks_jit_check.cu: the offline build / SASS check).
+// the marching CTAs (about half of all executed instructions with run-time geometry: round 1, see the history row of profiles/r3_kernels.md) folds away.
+// ugks_jit_check (include/ugks.h) compiles them for a geometry without a device: the offline build / SASS check.
 //
 // Notation follows DESIGN.md / include/ugks.h: cells (i,j), velocity point q = m*Nu + k, local face frame (n,t) = (u,v) on
 // x-faces and (v,u) on y-faces (AMB-21).
@@ -26,7 +26,7 @@ constexpr int FRS = G_FRS, CRS = G_CRS;                              // face / c
 constexpr int BCX0 = G_BC0, BCX1 = G_BC1, BCY0 = G_BC2, BCY1 = G_BC3;
 constexpr int NCHUNK = G_NCHUNK, MC = G_MC, R = G_R, NPT = G_NPT, STRIP = G_STRIP;
 constexpr int NSTRIP = (GI + STRIP - 1) / STRIP;
-constexpr int BT = ((NU * R + 31) / 32) * 32;                         // compute threads of a CTA; one more warp produces (TMA)
+constexpr int BT = ((NU * R + 31) / 32) * 32;                         // threads of a CTA: one per (column, parallel row); lane 0 of a rotating warp issues the bulk copies
 constexpr int KXM_END = G_KXM_END, KXP_BEGIN = G_KXP_BEGIN;          // columns with u_k <= 0: [0, KXM_END); u_k >= 0: [KXP_BEGIN, NU)
 constexpr int pad2c(int x) { return (x + 1) & ~1; }
 constexpr int QB = G_QB;                                              // doubles per staged chunk of a row: >= MC*NU + 1 (shift of an odd start), even;
@@ -148,8 +148,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
                  " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
                  " @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-// barrier among the compute threads only (the producer warp does not take part): bar.sync id, count
-__device__ __forceinline__ void bar_compute() { asm volatile("bar.sync 1, %0;" ::"n"(BT) : "memory"); }
 
 struct true_c { static constexpr bool value = true; };
 struct false_c { static constexpr bool value = false; };
@@ -165,20 +163,6 @@ __device__ __forceinline__ double vl_half(double dm, double dp)
     const double pr = dm * dp, s = dm + dp;
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(s));
-#if defined(UGKS_VL_SERIAL)                                          // round-2 form: refine r, then multiply (one level deeper)
-    const double e = fma(-s, r, 1.0);
-    const double t = fma(e, e, e);
-    r = fma(r, t, r);
-    const double hs = pr * r;
-#elif defined(UGKS_VL_NEWTON2)                                       // experiment: one Newton step on the quotient, error ~ 2^-46
-    const double q0 = pr * r;
-    const double hs = fma(fma(-s, q0, pr), r, q0);
-#elif defined(UGKS_VL_SELECT_RESULT)                                 // round-2 form: select the 64-bit result (two FSEL)
-    const double q0 = pr * r;
-    const double e = fma(-s, r, 1.0);
-    const double t = fma(e, e, e);
-    const double hs = fma(q0, t, q0);
-#else
     // q0 = pr r0 is formed beside e = 1 - s r0, so the chain after s is MUFU, e, t = e + e^2, q0 (1 + t): four deep, not five.
     // The sign test acts on the seed: its low word is zero by construction (MUFU.RCP64H), so "no slope" is one 32-bit select of
     // the high word; with r0 = 0 the chain gives q0 = 0, e = 1, t = 2, hs = fma(0, 2, 0) = 0 exactly.
@@ -187,8 +171,4 @@ __device__ __forceinline__ double vl_half(double dm, double dp)
     const double e = fma(-s, r, 1.0);
     const double t = fma(e, e, e);
     return fma(q0, t, q0);
-#endif
-#if defined(UGKS_VL_SERIAL) || defined(UGKS_VL_NEWTON2) || defined(UGKS_VL_SELECT_RESULT)
-    return __double2hiint(pr) > 0 ? hs : 0.0;
-#endif
 }

@@ -196,13 +196,11 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
         }
     }
     __syncthreads();
-    // the factors of a thread's stage-3 items never change along the march: short items keep them in registers (UGKS_S3REG doubles
+    // the factors of a thread's stage-3 items never change along the march: short items keep them in registers (S3REG doubles
     // at most), which halves the shared-memory loads of stage 3 -- the loads with most of this kernel's bank conflicts
-#ifndef UGKS_S3REG
-#define UGKS_S3REG 32
-#endif
+    constexpr int S3REG = 32;
     constexpr int S3LEN = cmaxi(L::PERX, L::PERY);
-    constexpr bool FREG = S3R * S3LEN <= UGKS_S3REG;
+    constexpr bool FREG = S3R * S3LEN <= S3REG;
     double itfac[FREG ? S3R * S3LEN : 1];
     if constexpr (FREG) {
 #pragma unroll
@@ -220,10 +218,6 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
     int qo[NPT];
 #pragma unroll
     for (int p = 0; p < NPT; ++p) qo[p] = r + p * R < mc ? p * QSTEP : qsh * 8 - qb0;
-#ifdef UGKS_TEST_STALE_READ                                          // negative control of the "poison" test
-#pragma unroll
-    for (int p = 0; p < NPT; ++p) qo[p] = p * QSTEP;
-#endif
 #define QOFF(p) ((G_RAGGED == 0 && ((p) + 1) * R <= MC) ? (p) * QSTEP : qo[p])
     const unsigned char *xring_b = reinterpret_cast<const unsigned char *>(xring);
     const unsigned char *ybuf_b = reinterpret_cast<const unsigned char *>(ybuf);
@@ -256,10 +250,8 @@ __device__ __forceinline__ void cell_moments_body(const KArgs &A, const int chun
 
     int xslot = 2 % NSXM, xphase = 2 / NSXM, ybuf_i = 0, yphase = 0; // ring slot / phase of row a+1 and of y stage a
     int issuer = 0;                                                  // lane 0 of a rotating warp issues the copies of a step
-#ifndef UGKS_UNROLL_M
-#define UGKS_UNROLL_M (STRIP >= 16 ? 2 : 1)                        // measured (C3, C4): -2 %; short strips: +10 %
-#endif
-#pragma unroll UGKS_UNROLL_M
+    constexpr int UNROLL_M = STRIP >= 16 ? 2 : 1;                    // measured (C3, C4): -2 %; short strips: +10 %
+#pragma unroll UNROLL_M
     for (int a = c0; a < c1 + LAG3 + 1; ++a) {
         if (a < c1) {                                                // stage 1: point sums of cell a
             mbar_wait(&bars[xslot], xphase);                         // row a+1
@@ -438,10 +430,6 @@ static_assert(MomL<true>::BYTES == G_SMEM_MOMX, "host mirror of the shared-memor
 static_assert(!TG, "the tangential reconstruction needs sorted velocity nodes (no mixed-sign chunks)");
 #endif
 
-#ifdef UGKS_MINB_MOM                                                // experiment override (UGKS_JIT_DEFS)
-#undef G_MINB_MOM
-#define G_MINB_MOM UGKS_MINB_MOM
-#endif
 extern "C" __global__ void __launch_bounds__(BT, G_MINB_MOM) k_cell_moments(const KArgs A, const int chunk0)
 {
     cell_moments_body<false>(A, chunk0);

@@ -199,10 +199,9 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
     int xw_slot = 0, xw_phase = 1;                                   // barrier slot / phase of row a+1 (index a+1-rows_first = 3 at a = c0)
     int stage_i = 0, stage_phase = 0;
     int issuer = 0;                                                  // thread that issues the bulk copies after this step (lane 0 of a rotating warp)
-#ifndef UGKS_UNROLL_U
-#define UGKS_UNROLL_U ((STRIP >= 16 && NU * R >= 128) ? 2 : 1)     // measured: C4 (160 threads) -10 % (the ring / stage parities and half of the register
-                                                                     // rotation fold away), C5 0; CTAs of 64-96 threads (C3, M4-69) +3 %, short strips +10 %
-#endif
+    // measured: C4 (160 threads) -10 % (the ring / stage parities and half of the register rotation fold away), C5 0; CTAs of
+    // 64-96 threads (C3, M4-69) +3 %, short strips +10 %
+    constexpr int UNROLL_U = (STRIP >= 16 && NU * R >= 128) ? 2 : 1;
     // one step: x-face a, then cell a-1.  The first step of a march (a = c0) has no cell to finish: it is peeled off (HC = false) so
     // that the steady-state body carries no "have a cell" branch between its points and the points of a thread form one basic block
     // (the independent FP64 chains of the NPT points can then be interleaved by the scheduler)
@@ -354,7 +353,7 @@ __device__ __forceinline__ void flux_update_body(const KArgs &A, const int4 ch, 
         if (issuer >= BT) issuer = 0;
     };
     step(c0, false_c{});
-#pragma unroll UGKS_UNROLL_U
+#pragma unroll UNROLL_U
     for (int a = c0 + 1; a <= c1; ++a) step(a, true_c{});
 }
 
@@ -365,28 +364,11 @@ static_assert(!TG, "the tangential reconstruction needs sorted velocity nodes (n
 
 // one launch covers the chunk range [chunk0, chunk0 + nch): the CTA dispatches on the sign class of its chunk (the two uniform
 // classes of a cell read its records while they are in the L2)
-#ifdef UGKS_MINB_UPD                                                // experiment override (UGKS_JIT_DEFS)
-#undef G_MINB_UPD
-#define G_MINB_UPD UGKS_MINB_UPD
-#endif
 extern "C" __global__ void __launch_bounds__(BT, G_MINB_UPD) k_flux_update(const KArgs A, const int chunk0)
 {
     int b = blockIdx.x;
-#ifndef UGKS_ORDER_U
-#define UGKS_ORDER_U 0
-#endif
-#if UGKS_ORDER_U == 1
-    // launch order: chunks fastest, then rows, then strips -- the CTAs that read the face and cell records of a cell (one per chunk)
-    // run together, so the records cross HBM once per step, and so do the y-neighbour rows (rows j-2 .. j+2 are in flight together)
-    const int c = b % NCHUNK; b /= NCHUNK;
-    const int j = b % GJ, s = b / GJ;
-#elif UGKS_ORDER_U == 2
-    const int j = b % GJ; b /= GJ;
-    const int c = b % NCHUNK, s = b / NCHUNK;
-#else
     const int j = b % GJ; b /= GJ;
     const int s = b % NSTRIP, c = b / NSTRIP;                        // rows fastest, then strips, then chunks
-#endif
     const int4 ch = c_chunks[chunk0 + c];
     if (ch.z > 0) flux_update_body<1>(A, ch, j, s);
     else if (ch.z < 0) flux_update_body<-1>(A, ch, j, s);

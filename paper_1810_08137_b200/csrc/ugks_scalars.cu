@@ -153,7 +153,7 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
         Tm[3] = iht * 0.5 * (raw[TGS ? RW_T31 : 0] + raw[TGS ? RW_T13 : 0]);
     }
     double *cf = P.frec[DIR] + face * P.frs, *fw = P.fw[DIR] + face * 4;
-    const double h = 0.5 * (DIR == 0 ? P.dx : P.dy), ell = DIR == 0 ? P.dy : P.dx, dt = P.dt;
+    const double ell = DIR == 0 ? P.dy : P.dx, dt = P.dt;
 
     double WL[4], WR[4], gL[4], gR[4];
     int kL, kR;
@@ -268,10 +268,7 @@ __device__ void face_scalars(const UgksParams &P, int cur, int pos, int line)
 }
 
 template <bool TGS>
-#ifndef UGKS_FS_MINB
-#define UGKS_FS_MINB 3
-#endif
-__global__ void __launch_bounds__(128, UGKS_FS_MINB) k_face_scalars(const UgksParams P, const int cur)
+__global__ void __launch_bounds__(128, 3) k_face_scalars(const UgksParams P, const int cur)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     const int nfx = nfaces_x(P), nfy = nfaces_y(P);
@@ -464,10 +461,7 @@ int launch_setup(const UgksParams &P, const double *bc_prims, double *ghost, dou
 // D_s = exp(-lam h (2 (x_s - c) + h)),  Q = exp(-2 lam h^2); seven steps add at most ~30 roundings (3e-15 relative; segments of 16 were
 // measured: no faster, and 1.3e-14 at the end of a segment breaks the fixed-point test's 1e-14).  Segments in
 // the far tail (E_s or D_s outside the normal range) and unequally spaced nodes take the direct exponentials.
-#ifndef UGKS_TSEG
-#define UGKS_TSEG 8
-#endif
-constexpr int TSEG = UGKS_TSEG;
+constexpr int TSEG = 8;
 __global__ void __launch_bounds__(256) k_tables(const UgksParams P, const unsigned TPB)      // TPB: tables per block pass (about 256 / segments per table)
 {
     const unsigned nsu = (P.NuP + TSEG - 1) / TSEG, nsv = (P.NvP + TSEG - 1) / TSEG, nseg = nsu + nsv;

@@ -50,7 +50,7 @@ def test_version_and_workspace_bytes(libugks):
     assert binding.workspace_bytes(bad) == 0
     # velocity grids: up to 512 columns (one thread per column of a CTA), not more
     import dataclasses
-    for nu, ok in ((256, True), (512, True), (513, False)):
+    for nu, ok in ((256, True), (512, True), (513, False)):                  # (Nv = 16 here)
         u, wu = workloads.trapezoid_grid(nu, 20.0)
         q = dataclasses.replace(workloads.channel_config("C1"), u=u, wu=wu)
         assert (binding.workspace_bytes(q) > 0) == ok, nu
@@ -78,6 +78,72 @@ def test_argument_validation_happens_before_cuda(libugks):
     assert init(ws=C.c_void_p(8)) == 1                                        # misaligned workspace
     assert libugks.ugks_step(None, 1) == 1 and libugks.ugks_sync(None) == 1
     assert libugks.ugks_dt(None) == 0.0 and libugks.ugks_step_count(None) == -1
+
+
+def test_velocity_grid_limits_and_non_finite_nodes(libugks):
+    """(1) a grid whose nodes, weights and chunk table overflow the 64 KB constant bank of the run-time compiled kernels
+    is refused by ugks_workspace_bytes already (it used to pass there and fail in NVRTC at ugks_init); the largest accepted
+    shapes do compile.  (2) NaN / Inf nodes or weights are UGKS_EINVAL before anything is compiled."""
+    import dataclasses
+    from paper_1810_08137_b200 import binding
+    base = workloads.channel_config("C1", I=8, J=4)
+
+    def grid(nu, nv):
+        u, wu = workloads.trapezoid_grid(nu, 20.0)
+        v, wv = workloads.trapezoid_grid(nv, 20.0)
+        return dataclasses.replace(base, u=u, wu=wu, v=v, wv=wv)
+
+    assert binding.workspace_bytes(grid(8, 2049)) == 0                        # Nv <= 2048
+    assert binding.workspace_bytes(grid(512, 2048)) == 0                      # 1-row chunks: 2048 x 16 B of chunk table on top of 40 KB of nodes
+    for nu, nv in ((8, 2048), (512, 1024)):
+        q = grid(nu, nv)
+        assert binding.workspace_bytes(q) > 0
+        binding.jit_check(q)                                                  # raises on a compile error
+    for field in ("u", "wu", "v", "wv"):
+        for bad in (float("nan"), float("inf")):
+            a = np.array(getattr(base, field), dtype=float)
+            a[3] = bad
+            q = dataclasses.replace(base, **{field: a})
+            with pytest.raises(binding.UgksError) as ei:
+                binding.jit_check(q)
+            assert ei.value.code == 1, (field, bad)
+            keep, mesh, vg, gas, bcs = binding._structs(q)
+            h = C.c_void_p()
+            rc = libugks.ugks_init(C.byref(h), C.byref(mesh), C.byref(vg), C.byref(gas), C.byref(bcs), 0.8, C.c_void_p(256), 1 << 40, None)
+            assert rc == 1 and b"finite" in libugks.ugks_last_error(None), (field, bad)
+
+
+def test_generated_source_does_not_depend_on_the_locale():
+    """the velocity nodes are written into the kernel source as hexadecimal literals built from their bits, so a host
+    application running under a comma-radix LC_NUMERIC still compiles (printf("%a") would have written 0x1,8p+1)."""
+    code = (
+        "import locale, sys\n"
+        "sys.path.insert(0, %r)\n"
+        "ok = False\n"
+        "for name in ('de_DE.UTF-8', 'de_DE.utf8', 'fr_FR.UTF-8', 'fr_FR.utf8', 'de_DE', 'fr_FR'):\n"
+        "    try:\n"
+        "        locale.setlocale(locale.LC_ALL, name); ok = True; break\n"
+        "    except locale.Error:\n"
+        "        pass\n"
+        "if not ok or locale.localeconv()['decimal_point'] != ',':\n"
+        "    print('NOLOCALE'); sys.exit(0)\n"
+        "import workloads\n"
+        "from paper_1810_08137_b200 import jit_check\n"
+        "jit_check(workloads.channel_config('C1'))\n"
+        "print('COMPILED')\n" % ROOT)
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    if "NOLOCALE" in r.stdout:
+        pytest.skip("no comma-radix locale installed on this machine")
+    assert "COMPILED" in r.stdout
+
+
+def test_shipped_library_reads_no_environment_variable(libugks):
+    """The experiment hooks (UGKS_JIT_DEFS pasted text into the kernel source) exist only in a -DUGKS_DEVELOPER build."""
+    from paper_1810_08137_b200 import binding
+    blob = open(binding.library_path(), "rb").read()
+    for name in (b"UGKS_JIT_DEFS", b"UGKS_NSXM", b"UGKS_SLICE", b"UGKS_JIT_MAXREG", b"UGKS_JIT_DUMP", b"UGKS_DEBUG", b"UGKS_JIT_CHECK_TANGENTIAL"):
+        assert name not in blob, name
 
 
 def test_product_package_does_not_touch_the_oracle():
